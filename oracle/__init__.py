@@ -1,0 +1,189 @@
+"""ctypes binding of the CPU oracle (oracle/exx_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this package.  It shares no code with paper_1712_07973_b200.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build as build_oracle
+
+_lib = None
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int)
+_lp = C.POINTER(C.c_longlong)
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build_oracle())
+        lib.exx_oracle_create.argtypes = [C.POINTER(C.c_void_p), _ip, _dp, C.c_int, _dp]
+        lib.exx_oracle_destroy.argtypes = [C.c_void_p]
+        lib.exx_oracle_destroy.restype = None
+        lib.exx_oracle_fft1d.argtypes = [C.c_int, _dp, C.c_int]
+        lib.exx_oracle_transform_dims.argtypes = [C.c_void_p, _ip]
+        lib.exx_oracle_transform_dims.restype = None
+        lib.exx_oracle_get_khat.argtypes = [C.c_void_p, _dp]
+        lib.exx_oracle_poisson.argtypes = [C.c_void_p, _dp, _dp]
+        lib.exx_oracle_apply.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_int]
+        lib.exx_oracle_rows.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int, _ip, _dp, _dp]
+        lib.exx_oracle_pair_energies.argtypes = [C.c_void_p, C.c_int, _dp, C.c_int, _ip, _ip, _dp]
+        lib.exx_oracle_realspace_kernel.argtypes = [C.c_void_p, _dp]
+        lib.exx_oracle_poisson_direct.argtypes = [C.c_void_p, _dp, _dp]
+        lib.exx_oracle_kpsi_points.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int, _ip, _lp, _dp]
+        lib.exx_oracle_threads.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def fft1d(x, sign=-1):
+    """Unnormalised 1-D DFT by the oracle's own FFT (complex128 in, complex128 out)."""
+    z = np.ascontiguousarray(np.asarray(x, dtype=np.complex128)).copy()
+    buf = z.view(np.float64)
+    rc = _load().exx_oracle_fft1d(int(z.size), _d(buf), int(sign))
+    if rc:
+        raise RuntimeError(f"exx_oracle_fft1d failed ({rc})")
+    return z
+
+
+class Oracle:
+    """Plain CPU exact-exchange oracle for one grid / boundary condition / Green's function."""
+
+    def __init__(self, dims, spacing, bc, kernel=None):
+        lib = _load()
+        self.dims = tuple(int(d) for d in dims)
+        self.spacing = tuple(float(h) for h in spacing)
+        self.bc = {"periodic": 0, "free": 1}[bc] if isinstance(bc, str) else int(bc)
+        self.M = self.dims[0] * self.dims[1] * self.dims[2]
+        self.dV = self.spacing[0] * self.spacing[1] * self.spacing[2]
+        d = (C.c_int * 3)(*self.dims)
+        h = (C.c_double * 3)(*self.spacing)
+        k = None
+        if kernel is not None:
+            k = _f64(kernel)
+            if k.size != self.M:
+                raise ValueError("kernel table must have n1*n2*n3 entries")
+        self._h = C.c_void_p()
+        rc = lib.exx_oracle_create(C.byref(self._h), d, h, self.bc, _d(k) if k is not None else None)
+        if rc:
+            raise RuntimeError(f"exx_oracle_create failed ({rc})")
+        t = (C.c_int * 3)()
+        lib.exx_oracle_transform_dims(self._h, t)
+        self.tdims = tuple(t)
+
+    def close(self):
+        if self._h:
+            _load().exx_oracle_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def khat(self):
+        out = np.empty(self.tdims, dtype=np.complex128)
+        rc = _load().exx_oracle_get_khat(self._h, _d(out.view(np.float64)))
+        if rc:
+            raise RuntimeError("exx_oracle_get_khat failed")
+        return out
+
+    def poisson(self, rho):
+        rho = _f64(rho).reshape(self.dims)
+        v = np.empty(self.dims)
+        rc = _load().exx_oracle_poisson(self._h, _d(rho), _d(v))
+        if rc:
+            raise RuntimeError("exx_oracle_poisson failed")
+        return v
+
+    def poisson_direct(self, rho):
+        rho = _f64(rho).reshape(self.dims)
+        v = np.empty(self.dims)
+        rc = _load().exx_oracle_poisson_direct(self._h, _d(rho), _d(v))
+        if rc:
+            raise RuntimeError("exx_oracle_poisson_direct failed")
+        return v
+
+    def realspace_kernel(self):
+        g = np.empty(self.dims)
+        rc = _load().exx_oracle_realspace_kernel(self._h, _d(g))
+        if rc:
+            raise RuntimeError("exx_oracle_realspace_kernel failed")
+        return g
+
+    def apply(self, psi, occ, symmetric=False):
+        """Returns (kpsi[N,n1,n2,n3], E_x, e_pair[N,N])."""
+        psi = _f64(psi)
+        n_orb = psi.shape[0]
+        psi = psi.reshape(n_orb, self.M)
+        occ = _f64(occ)
+        kpsi = np.empty_like(psi)
+        ex = C.c_double()
+        e = np.empty((n_orb, n_orb))
+        rc = _load().exx_oracle_apply(self._h, n_orb, _d(psi), _d(occ), _d(kpsi), C.byref(ex), _d(e),
+                                      1 if symmetric else 0)
+        if rc:
+            raise RuntimeError(f"exx_oracle_apply failed ({rc})")
+        return kpsi.reshape((n_orb,) + self.dims), ex.value, e
+
+    def rows(self, psi, occ, rows):
+        """Complete rows K psi_i for listed i: returns (kpsi_rows[len(rows),n1,n2,n3], e_rows[len(rows),N])."""
+        psi = _f64(psi)
+        n_orb = psi.shape[0]
+        psi = psi.reshape(n_orb, self.M)
+        occ = _f64(occ)
+        rows = np.ascontiguousarray(np.asarray(rows, dtype=np.int32))
+        out = np.empty((rows.size, self.M))
+        e = np.empty((rows.size, n_orb))
+        rc = _load().exx_oracle_rows(self._h, n_orb, _d(psi), _d(occ), int(rows.size),
+                                     rows.ctypes.data_as(_ip), _d(out), _d(e))
+        if rc:
+            raise RuntimeError(f"exx_oracle_rows failed ({rc})")
+        return out.reshape((rows.size,) + self.dims), e
+
+    def pair_energies(self, psi, pairs):
+        psi = _f64(psi)
+        n_orb = psi.shape[0]
+        psi = psi.reshape(n_orb, self.M)
+        pairs = np.asarray(pairs, dtype=np.int32).reshape(-1, 2)
+        pi = np.ascontiguousarray(pairs[:, 0])
+        pj = np.ascontiguousarray(pairs[:, 1])
+        e = np.empty(pairs.shape[0])
+        rc = _load().exx_oracle_pair_energies(self._h, n_orb, _d(psi), int(e.size), pi.ctypes.data_as(_ip),
+                                              pj.ctypes.data_as(_ip), _d(e))
+        if rc:
+            raise RuntimeError(f"exx_oracle_pair_energies failed ({rc})")
+        return e
+
+    def kpsi_points(self, psi, occ, orbs, points):
+        """Sampled K psi entries by direct real-space summation (no FFT in the convolution)."""
+        psi = _f64(psi)
+        n_orb = psi.shape[0]
+        psi = psi.reshape(n_orb, self.M)
+        occ = _f64(occ)
+        orbs = np.ascontiguousarray(np.asarray(orbs, dtype=np.int32))
+        points = np.ascontiguousarray(np.asarray(points, dtype=np.int64))
+        out = np.empty(orbs.size)
+        rc = _load().exx_oracle_kpsi_points(self._h, n_orb, _d(psi), _d(occ), int(orbs.size),
+                                            orbs.ctypes.data_as(_ip), points.ctypes.data_as(_lp), _d(out))
+        if rc:
+            raise RuntimeError(f"exx_oracle_kpsi_points failed ({rc})")
+        return out
+
+
+def threads_used() -> int:
+    return int(_load().exx_oracle_threads())
