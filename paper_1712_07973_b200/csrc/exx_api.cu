@@ -1,0 +1,598 @@
+// exx_api.cu -- plan, tables, pair scheduling and the C ABI of libexx_b200 (include/exx.h).
+//
+// Hot path per same-i batch (PAPER.md:113-117 kernels 1-3, fused): pass A -> pass B -> pass C -> energy reduce,
+// all enqueued on the plan's stream; the host only schedules.  No CPU fallback exists anywhere in this file:
+// without a usable CUDA device every computing entry point returns EXX_ERR_CUDA.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/exx.h"
+#include "exx_launch.h"
+#include "exx_sched.hpp"
+
+using namespace exx;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+
+// ------------------------------------------------------------------------------------------ small kernels
+
+// Periodic Fourier-space kernel on the symmetric index range s = 0..T/2 per axis (m = s):
+// K^ = 4 pi / |G|^2, G = 2 pi (m1/(t1 h1), m2/(t2 h2), m3/(t3 h3)), K^(0) = 0; times 1/T_tot (inverse FFT norm).
+__global__ void ks_periodic_kernel(double* ks, int na, int nb, int nc, double ga, double gb, double gc, double scale) {
+    const long long total = static_cast<long long>(na) * nb * nc;
+    for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
+         x += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int sc = static_cast<int>(x % nc);
+        const int sb = static_cast<int>((x / nc) % nb);
+        const int sa = static_cast<int>(x / (static_cast<long long>(nc) * nb));
+        const double g1 = ga * sa, g2 = gb * sb, g3 = gc * sc;
+        const double gg = g1 * g1 + g2 * g2 + g3 * g3;
+        ks[x] = (x == 0) ? 0.0 : scale * 4.0 * kPi / gg;
+    }
+}
+
+// g'[a][b][c] = g[a][b][c] * (1/2 per zero index): folds the even mirror extension of the Hockney kernel.
+__global__ void halve_origin_planes_kernel(double* g, int na, int nb, int nc) {
+    const long long total = static_cast<long long>(na) * nb * nc;
+    for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
+         x += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int c = static_cast<int>(x % nc);
+        const int b = static_cast<int>((x / nc) % nb);
+        const int a = static_cast<int>(x / (static_cast<long long>(nc) * nb));
+        double f = 1.0;
+        if (a == 0) f *= 0.5;
+        if (b == 0) f *= 0.5;
+        if (c == 0) f *= 0.5;
+        g[x] *= f;
+    }
+}
+
+// out[o][k][i] = scale * sum_a 2 cos(2 pi a k / T) in[o][a][i],  k = 0..n_out-1  (one axis of the DFT of the
+// even extension g_ext of the free-BC table; the index-n plane of g_ext is zero, reading A8).
+__global__ void cos_transform_kernel(const double* in, double* out, long long outer, int n_in, int n_out, long long inner,
+                                     int T, double scale) {
+    const long long total = outer * n_out * inner;
+    for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
+         x += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long i = x % inner;
+        const int k = static_cast<int>((x / inner) % n_out);
+        const long long o = x / (inner * n_out);
+        const double* src = in + o * n_in * inner + i;
+        double s = 0.0, comp = 0.0;
+        for (int a = 0; a < n_in; ++a) {
+            const int m = static_cast<int>((static_cast<long long>(a) * k) % T);
+            const double term = 2.0 * cospi(2.0 * m / T) * src[a * inner];
+            const double y = term - comp;                 // Kahan
+            const double t = s + y;
+            comp = (t - s) - y;
+            s = t;
+        }
+        out[x] = scale * s;
+    }
+}
+
+// e_ij = dV * sum over tiles of the per-CTA partial sums of pass C, fixed order (deterministic).
+__global__ void reduce_energy_kernel(const double* epart, int tiles, const XformDesc* desc, int i, int n_orb, double dV,
+                                     double* e_mat) {
+    __shared__ double sh[2][256];
+    const int t = blockIdx.x;
+    const double* ep = epart + static_cast<size_t>(t) * tiles * 2;
+    double s1 = 0.0, s2 = 0.0;
+    for (int k = threadIdx.x; k < tiles; k += blockDim.x) { s1 += ep[2 * k]; s2 += ep[2 * k + 1]; }
+    sh[0][threadIdx.x] = s1; sh[1][threadIdx.x] = s2;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) { sh[0][threadIdx.x] += sh[0][threadIdx.x + o]; sh[1][threadIdx.x] += sh[1][threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const XformDesc d = desc[t];
+        const double e1 = dV * sh[0][0];
+        e_mat[static_cast<size_t>(i) * n_orb + d.j] = e1;
+        e_mat[static_cast<size_t>(d.j) * n_orb + i] = e1;
+        if (d.l >= 0) {
+            const double e2 = dV * sh[1][0];
+            e_mat[static_cast<size_t>(i) * n_orb + d.l] = e2;
+            e_mat[static_cast<size_t>(d.l) * n_orb + i] = e2;
+        }
+    }
+}
+
+// E_x = -1/2 sum_{i,j} f_i f_j e_ij over ordered pairs (Eq. 5), fixed-order tree.
+__global__ void exchange_energy_kernel(const double* e_mat, const double* occ, int n_orb, double* ex) {
+    __shared__ double sh[1024];
+    const long long total = static_cast<long long>(n_orb) * n_orb;
+    double s = 0.0;
+    for (long long x = threadIdx.x; x < total; x += blockDim.x) {
+        const int i = static_cast<int>(x / n_orb), j = static_cast<int>(x % n_orb);
+        s += occ[i] * occ[j] * e_mat[x];
+    }
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *ex = -0.5 * sh[0];
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------ plan
+struct exx_plan {
+    int n[3], t[3];
+    double h[3];
+    double dV;
+    int bc;
+    long long M;
+    Geometry geo;
+    int max_orb;
+    int max_batch;
+    cudaStream_t stream;
+    double2* tw[3];
+    double2* roots[3];
+    double* ks;
+    double2* w1;
+    size_t w1_elems_per_xform;
+    double* epart;
+    double* e_mat;
+    double* occ_dev;
+    XformDesc* desc_dev;
+    size_t desc_cap;
+    XformDesc* desc_pinned;
+    double* occ_pinned;
+    double* ex_dev;
+    double* ex_pinned;
+    cudaEvent_t upload_done;
+    double* psi_stage;
+    double* kpsi_stage;
+    size_t stage_elems;
+    KernelInfo info_ac, info_b;
+    long long launches;
+    int last_n_orb;
+    size_t ws_bytes;        // batch workspace (W1 + energy partials)
+    size_t fixed_bytes;     // tables, descriptors, pair-energy matrix
+    std::string err;
+};
+
+namespace {
+
+exx_status fail(exx_plan* p, exx_status s, const std::string& msg) {
+    if (p) p->err = msg; else g_create_error = msg;
+    return s;
+}
+
+exx_status cuda_fail(exx_plan* p, cudaError_t e, const char* what) {
+    std::string msg = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+    cudaGetLastError();
+    return fail(p, EXX_ERR_CUDA, msg);
+}
+
+#define EXX_CUDA(plan, call)                                             \
+    do {                                                                 \
+        cudaError_t e__ = (call);                                        \
+        if (e__ != cudaSuccess) return cuda_fail(plan, e__, #call);      \
+    } while (0)
+
+bool is_device_pointer(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// [k1*Q + n2] = W_T^{n2 k1};  roots[m] = W_T^m.  long double trigonometry, rounded once (no recurrences).
+void host_tables(int T, std::vector<double2>& tw, std::vector<double2>& roots) {
+    int P = 0, Q = 0;
+    switch (T) {
+        case 16: P = Split<16>::P; Q = Split<16>::Q; break;
+        case 32: P = Split<32>::P; Q = Split<32>::Q; break;
+        case 64: P = Split<64>::P; Q = Split<64>::Q; break;
+        case 96: P = Split<96>::P; Q = Split<96>::Q; break;
+        case 128: P = Split<128>::P; Q = Split<128>::Q; break;
+        case 192: P = Split<192>::P; Q = Split<192>::Q; break;
+        case 256: P = Split<256>::P; Q = Split<256>::Q; break;
+        default: break;
+    }
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    roots.resize(T);
+    for (int m = 0; m < T; ++m) {
+        const long double ang = two_pi * m / T;
+        roots[m] = make_double2(static_cast<double>(cosl(ang)), static_cast<double>(-sinl(ang)));
+    }
+    tw.resize(T);
+    for (int k1 = 0; k1 < P; ++k1)
+        for (int n2 = 0; n2 < Q; ++n2) tw[k1 * Q + n2] = roots[(k1 * n2) % T];
+}
+
+void split_of(int T, int* P, int* Q) {
+    std::vector<double2> a, b;
+    (void)a; (void)b;
+    switch (T) {
+        case 16: *P = Split<16>::P; *Q = Split<16>::Q; break;
+        case 32: *P = Split<32>::P; *Q = Split<32>::Q; break;
+        case 64: *P = Split<64>::P; *Q = Split<64>::Q; break;
+        case 96: *P = Split<96>::P; *Q = Split<96>::Q; break;
+        case 128: *P = Split<128>::P; *Q = Split<128>::Q; break;
+        case 192: *P = Split<192>::P; *Q = Split<192>::Q; break;
+        default: *P = Split<256>::P; *Q = Split<256>::Q; break;
+    }
+}
+
+void free_workspace(exx_plan* p) {
+    if (p->w1) cudaFree(p->w1);
+    if (p->epart) cudaFree(p->epart);
+    p->w1 = nullptr;
+    p->epart = nullptr;
+}
+
+exx_status alloc_workspace(exx_plan* p, int max_batch) {
+    free_workspace(p);
+    p->max_batch = max_batch;
+    const size_t w1_bytes = p->w1_elems_per_xform * sizeof(double2) * static_cast<size_t>(max_batch);
+    const size_t ep_bytes = static_cast<size_t>(max_batch) * p->info_ac.tiles * 2 * sizeof(double);
+    cudaError_t e = cudaMalloc(&p->w1, w1_bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(p, EXX_ERR_ALLOC, "cudaMalloc(workspace W1) failed"); }
+    e = cudaMalloc(&p->epart, ep_bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(p, EXX_ERR_ALLOC, "cudaMalloc(energy partials) failed"); }
+    p->ws_bytes = w1_bytes + ep_bytes;
+    return EXX_OK;
+}
+
+int default_batch(const exx_plan* p) {
+    const double per = static_cast<double>(p->w1_elems_per_xform) * sizeof(double2);
+    long long b = static_cast<long long>(4.0 * 1024 * 1024 * 1024 / per);
+    if (b < 1) b = 1;
+    if (b > 64) b = 64;
+    return static_cast<int>(b);
+}
+
+exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
+    const int na = p->t[0] / 2 + 1, nb = p->t[1] / 2 + 1, nc = p->t[2] / 2 + 1;
+    const size_t total = static_cast<size_t>(na) * nb * nc;
+    if (cudaMalloc(&p->ks, total * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(p, EXX_ERR_ALLOC, "cudaMalloc(Fourier kernel) failed");
+    }
+    const double t_tot = static_cast<double>(p->t[0]) * p->t[1] * p->t[2];
+    const int threads = 256;
+    if (p->bc == EXX_BC_PERIODIC) {
+        const int blocks = static_cast<int>((total + threads - 1) / threads < 4096 ? (total + threads - 1) / threads : 4096);
+        ks_periodic_kernel<<<blocks, threads, 0, p->stream>>>(p->ks, na, nb, nc, 2.0 * kPi / (p->t[0] * p->h[0]),
+                                                              2.0 * kPi / (p->t[1] * p->h[1]),
+                                                              2.0 * kPi / (p->t[2] * p->h[2]), 1.0 / t_tot);
+        EXX_CUDA(p, cudaGetLastError());
+        ++p->launches;
+        EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+        return EXX_OK;
+    }
+    // FREE: K^ = dV * DFT3(g_ext) restricted to the symmetric index range, computed as three cosine transforms of
+    // g' (even extension folded); 1/T_tot of the inverse transform folded in.
+    const int n0 = p->n[0], n1 = p->n[1], n2 = p->n[2];
+    double *g = nullptr, *t1 = nullptr, *t2 = nullptr;
+    const size_t gsz = static_cast<size_t>(n0) * n1 * n2;
+    const size_t t1sz = static_cast<size_t>(na) * n1 * n2;
+    const size_t t2sz = static_cast<size_t>(na) * nb * n2;
+    if (cudaMalloc(&g, gsz * sizeof(double)) != cudaSuccess || cudaMalloc(&t1, t1sz * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&t2, t2sz * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        if (g) cudaFree(g);
+        if (t1) cudaFree(t1);
+        if (t2) cudaFree(t2);
+        return fail(p, EXX_ERR_ALLOC, "cudaMalloc(kernel table scratch) failed");
+    }
+    cudaError_t e = cudaMemcpyAsync(g, kernel_host, gsz * sizeof(double), cudaMemcpyHostToDevice, p->stream);
+    auto blocks_for = [&](size_t n) { size_t b = (n + threads - 1) / threads; return static_cast<int>(b < 8192 ? b : 8192); };
+    if (e == cudaSuccess) {
+        halve_origin_planes_kernel<<<blocks_for(gsz), threads, 0, p->stream>>>(g, n0, n1, n2);
+        cos_transform_kernel<<<blocks_for(t1sz), threads, 0, p->stream>>>(g, t1, 1, n0, na, static_cast<long long>(n1) * n2,
+                                                                          p->t[0], 1.0);
+        cos_transform_kernel<<<blocks_for(t2sz), threads, 0, p->stream>>>(t1, t2, na, n1, nb, n2, p->t[1], 1.0);
+        cos_transform_kernel<<<blocks_for(total), threads, 0, p->stream>>>(t2, p->ks, static_cast<long long>(na) * nb, n2, nc, 1,
+                                                                           p->t[2], p->dV / t_tot);
+        p->launches += 4;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    cudaFree(g); cudaFree(t1); cudaFree(t2);
+    if (e != cudaSuccess) return cuda_fail(p, e, "building the free-BC Fourier kernel");
+    return EXX_OK;
+}
+
+exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* occ_host, double* kpsi) {
+    // wait until the previous apply's descriptor upload has left the pinned staging buffers
+    EXX_CUDA(p, cudaEventSynchronize(p->upload_done));
+    Schedule sched = build_schedule(n_orb, occ_host, p->max_batch);
+    if (sched.xforms.size() > p->desc_cap) return fail(p, EXX_ERR_INTERNAL, "descriptor capacity exceeded");
+    if (!sched.xforms.empty()) std::memcpy(p->desc_pinned, sched.xforms.data(), sched.xforms.size() * sizeof(XformDesc));
+    std::memcpy(p->occ_pinned, occ_host, sizeof(double) * n_orb);
+    cudaStream_t s = p->stream;
+    if (!sched.xforms.empty())
+        EXX_CUDA(p, cudaMemcpyAsync(p->desc_dev, p->desc_pinned, sched.xforms.size() * sizeof(XformDesc), cudaMemcpyHostToDevice, s));
+    EXX_CUDA(p, cudaMemcpyAsync(p->occ_dev, p->occ_pinned, sizeof(double) * n_orb, cudaMemcpyHostToDevice, s));
+    EXX_CUDA(p, cudaEventRecord(p->upload_done, s));
+    EXX_CUDA(p, cudaMemsetAsync(kpsi, 0, sizeof(double) * static_cast<size_t>(n_orb) * p->M, s));
+    EXX_CUDA(p, cudaMemsetAsync(p->e_mat, 0, sizeof(double) * static_cast<size_t>(n_orb) * n_orb, s));
+
+    ArgsAC ac{};
+    ac.psi = psi; ac.kpsi = kpsi; ac.w1 = p->w1; ac.twc = p->tw[2]; ac.rootsb = p->roots[1]; ac.epart = p->epart;
+    ac.m_points = p->M; ac.na = p->n[0]; ac.chunk_log2 = p->geo.chunk_log2;
+    ArgsB ab{};
+    ab.w1 = p->w1; ab.twa = p->tw[0]; ab.ks = p->ks; ab.tc = p->t[2];
+    split_of(p->t[2], &ab.pc, &ab.qc);
+    ab.npch = p->t[2] >> p->geo.chunk_log2;
+
+    for (const Batch& b : sched.batches) {
+        ac.desc = p->desc_dev + b.first;
+        ac.i = b.i; ac.fi = occ_host[b.i]; ac.count = b.count;
+        EXX_CUDA(p, launch_pass_a(p->geo, ac, b.count, s, nullptr));
+        EXX_CUDA(p, launch_pass_b(p->geo, ab, b.count, s, nullptr));
+        EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
+        reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_ac.tiles, ac.desc, b.i, n_orb, p->dV, p->e_mat);
+        EXX_CUDA(p, cudaGetLastError());
+        p->launches += 4;
+    }
+    exchange_energy_kernel<<<1, 1024, 0, s>>>(p->e_mat, p->occ_dev, n_orb, p->ex_dev);
+    EXX_CUDA(p, cudaGetLastError());
+    ++p->launches;
+    p->last_n_orb = n_orb;
+    return EXX_OK;
+}
+
+exx_status check_apply_args(exx_plan* p, int n_orb, const void* psi, const double* occ, const void* kpsi, const void* ex) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    if (!psi || !occ || !kpsi || !ex) return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
+    if (n_orb < 1 || n_orb > p->max_orb) return fail(p, EXX_ERR_INVALID_ARG, "n_orb outside [1, max_orbitals]");
+    return EXX_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+const char* exx_version(void) { return "exx-b200 0.1 (sm_100a)"; }
+
+const char* exx_status_string(exx_status s) {
+    switch (s) {
+        case EXX_OK: return "EXX_OK";
+        case EXX_ERR_INVALID_ARG: return "EXX_ERR_INVALID_ARG";
+        case EXX_ERR_UNSUPPORTED_SIZE: return "EXX_ERR_UNSUPPORTED_SIZE";
+        case EXX_ERR_BAD_POINTER: return "EXX_ERR_BAD_POINTER";
+        case EXX_ERR_ALLOC: return "EXX_ERR_ALLOC";
+        case EXX_ERR_CUDA: return "EXX_ERR_CUDA";
+        case EXX_ERR_INTERNAL: return "EXX_ERR_INTERNAL";
+    }
+    return "EXX_ERR_UNKNOWN";
+}
+
+const char* exx_last_error(const exx_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+exx_status exx_schedule_pairs(int n_orb, const double* occ_host, long long* n_pairs, long long* n_transforms) {
+    if (n_orb < 1 || !occ_host || !n_pairs || !n_transforms) return EXX_ERR_INVALID_ARG;
+    try {
+        Schedule s = build_schedule(n_orb, occ_host, 1 << 30);
+        *n_pairs = s.n_pairs;
+        *n_transforms = static_cast<long long>(s.xforms.size());
+    } catch (const std::bad_alloc&) {
+        return EXX_ERR_ALLOC;
+    }
+    return EXX_OK;
+}
+
+exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spacing[3], exx_bc bc, const double* kernel_host,
+                           int max_orbitals, void* cuda_stream) {
+    g_create_error.clear();
+    if (!plan || !dims || !spacing) return fail(nullptr, EXX_ERR_INVALID_ARG, "NULL argument");
+    *plan = nullptr;
+    if (bc != EXX_BC_PERIODIC && bc != EXX_BC_FREE) return fail(nullptr, EXX_ERR_INVALID_ARG, "unknown boundary condition");
+    if (bc == EXX_BC_FREE && !kernel_host) return fail(nullptr, EXX_ERR_INVALID_ARG, "free BC needs a kernel table");
+    if (bc == EXX_BC_PERIODIC && kernel_host) return fail(nullptr, EXX_ERR_INVALID_ARG, "periodic BC takes no kernel table");
+    if (max_orbitals < 1) return fail(nullptr, EXX_ERR_INVALID_ARG, "max_orbitals < 1");
+    for (int ax = 0; ax < 3; ++ax) {
+        if (dims[ax] < 1) return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE, "non-positive grid length");
+        if (!(spacing[ax] > 0.0) || !std::isfinite(spacing[ax])) return fail(nullptr, EXX_ERR_INVALID_ARG, "spacing must be > 0");
+    }
+    Geometry geo{};
+    geo.free_bc = bc == EXX_BC_FREE ? 1 : 0;
+    geo.ta = geo.free_bc ? 2 * dims[0] : dims[0];
+    geo.tb = geo.free_bc ? 2 * dims[1] : dims[1];
+    geo.tc = geo.free_bc ? 2 * dims[2] : dims[2];
+    if (!geometry_supported(geo))
+        return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE,
+                    "transform lengths must be in {16,32,64,96,128,192,256}; non-cubic grids only with lengths <= 64");
+    geo.chunk_log2 = default_chunk_log2(geo.ta, geo.tb);
+
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, EXX_ERR_CUDA, std::string("no usable CUDA device: ") + (ce != cudaSuccess ? cudaGetErrorName(ce) : "device count 0"));
+    }
+    if (kernel_host && is_device_pointer(kernel_host))
+        return fail(nullptr, EXX_ERR_BAD_POINTER, "kernel_host must be a host pointer");
+
+    exx_plan* p = new (std::nothrow) exx_plan();
+    if (!p) return fail(nullptr, EXX_ERR_ALLOC, "out of host memory");
+    p->bc = bc;
+    p->geo = geo;
+    p->dV = 1.0;
+    p->M = 1;
+    for (int ax = 0; ax < 3; ++ax) {
+        p->n[ax] = dims[ax];
+        p->h[ax] = spacing[ax];
+        p->dV *= spacing[ax];
+        p->M *= dims[ax];
+    }
+    p->t[0] = geo.ta; p->t[1] = geo.tb; p->t[2] = geo.tc;
+    p->max_orb = max_orbitals;
+    p->stream = static_cast<cudaStream_t>(cuda_stream);
+
+    auto bail = [&](exx_status st) {
+        g_create_error = p->err;
+        exx_plan_destroy(p);
+        return st;
+    };
+    if (query_pass_ac(geo, &p->info_ac) != cudaSuccess || query_pass_b(geo, &p->info_b) != cudaSuccess)
+        return bail(fail(p, EXX_ERR_INTERNAL, "no kernel instantiation for this geometry"));
+
+    for (int ax = 0; ax < 3; ++ax) {
+        std::vector<double2> tw, roots;
+        host_tables(p->t[ax], tw, roots);
+        const size_t bytes = sizeof(double2) * p->t[ax];
+        if (cudaMalloc(&p->tw[ax], bytes) != cudaSuccess || cudaMalloc(&p->roots[ax], bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(p, EXX_ERR_ALLOC, "cudaMalloc(twiddles) failed"));
+        }
+        if (cudaMemcpy(p->tw[ax], tw.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(p->roots[ax], roots.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(p, EXX_ERR_CUDA, "twiddle upload failed"));
+        }
+    }
+    exx_status st = build_fourier_kernel(p, kernel_host);
+    if (st != EXX_OK) return bail(st);
+
+    p->w1_elems_per_xform = static_cast<size_t>(p->n[0]) * p->t[1] * p->t[2];
+    st = alloc_workspace(p, default_batch(p));
+    if (st != EXX_OK) return bail(st);
+
+    const size_t n = static_cast<size_t>(max_orbitals);
+    p->desc_cap = n * (n + 3) / 4 + n + 4;
+    bool ok = cudaMalloc(&p->e_mat, n * n * sizeof(double)) == cudaSuccess &&
+              cudaMalloc(&p->occ_dev, n * sizeof(double)) == cudaSuccess &&
+              cudaMalloc(&p->desc_dev, p->desc_cap * sizeof(XformDesc)) == cudaSuccess &&
+              cudaMalloc(&p->ex_dev, sizeof(double)) == cudaSuccess &&
+              cudaMallocHost(&p->desc_pinned, p->desc_cap * sizeof(XformDesc)) == cudaSuccess &&
+              cudaMallocHost(&p->occ_pinned, n * sizeof(double)) == cudaSuccess &&
+              cudaMallocHost(&p->ex_pinned, sizeof(double)) == cudaSuccess &&
+              cudaEventCreateWithFlags(&p->upload_done, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        return bail(fail(p, EXX_ERR_ALLOC, "allocation of plan buffers failed"));
+    }
+    p->fixed_bytes = n * n * sizeof(double) + n * sizeof(double) + p->desc_cap * sizeof(XformDesc) +
+                     sizeof(double) * (static_cast<size_t>(p->t[0] / 2 + 1) * (p->t[1] / 2 + 1) * (p->t[2] / 2 + 1));
+    if (cudaMemset(p->e_mat, 0, n * n * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        return bail(fail(p, EXX_ERR_CUDA, "cudaMemset failed"));
+    }
+    *plan = p;
+    return EXX_OK;
+}
+
+exx_status exx_plan_destroy(exx_plan* p) {
+    if (!p) return EXX_OK;
+    if (p->stream || p->w1) cudaStreamSynchronize(p->stream);
+    for (int ax = 0; ax < 3; ++ax) {
+        if (p->tw[ax]) cudaFree(p->tw[ax]);
+        if (p->roots[ax]) cudaFree(p->roots[ax]);
+    }
+    if (p->ks) cudaFree(p->ks);
+    free_workspace(p);
+    if (p->e_mat) cudaFree(p->e_mat);
+    if (p->occ_dev) cudaFree(p->occ_dev);
+    if (p->desc_dev) cudaFree(p->desc_dev);
+    if (p->ex_dev) cudaFree(p->ex_dev);
+    if (p->desc_pinned) cudaFreeHost(p->desc_pinned);
+    if (p->occ_pinned) cudaFreeHost(p->occ_pinned);
+    if (p->ex_pinned) cudaFreeHost(p->ex_pinned);
+    if (p->upload_done) cudaEventDestroy(p->upload_done);
+    if (p->psi_stage) cudaFree(p->psi_stage);
+    if (p->kpsi_stage) cudaFree(p->kpsi_stage);
+    cudaGetLastError();
+    delete p;
+    return EXX_OK;
+}
+
+exx_status exx_plan_transform_dims(const exx_plan* p, int tdims[3]) {
+    if (!p || !tdims) return EXX_ERR_INVALID_ARG;
+    for (int ax = 0; ax < 3; ++ax) tdims[ax] = p->t[ax];
+    return EXX_OK;
+}
+
+size_t exx_plan_workspace_bytes(const exx_plan* p) { return p ? p->ws_bytes + p->fixed_bytes : 0; }
+
+long long exx_plan_launch_count(const exx_plan* p) { return p ? p->launches : 0; }
+
+exx_status exx_plan_set_batch(exx_plan* p, int max_transforms_per_batch) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    int b = max_transforms_per_batch > 0 ? max_transforms_per_batch : default_batch(p);
+    if (b > 4096) b = 4096;
+    return alloc_workspace(p, b);
+}
+
+exx_status exx_apply_async(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, double* kpsi_dev, double* ex_dev) {
+    exx_status st = check_apply_args(p, n_orb, psi_dev, occ_host, kpsi_dev, ex_dev);
+    if (st != EXX_OK) return st;
+    if (!is_device_pointer(psi_dev) || !is_device_pointer(kpsi_dev) || !is_device_pointer(ex_dev))
+        return fail(p, EXX_ERR_BAD_POINTER, "psi_dev, kpsi_dev and ex_dev must be device pointers");
+    if (is_device_pointer(occ_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host must be a host pointer");
+    if (psi_dev == kpsi_dev) return fail(p, EXX_ERR_INVALID_ARG, "kpsi must not alias psi");
+    st = apply_impl(p, n_orb, psi_dev, occ_host, kpsi_dev);
+    if (st != EXX_OK) return st;
+    EXX_CUDA(p, cudaMemcpyAsync(ex_dev, p->ex_dev, sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
+    return EXX_OK;
+}
+
+exx_status exx_apply(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, double* kpsi_dev, double* ex_host) {
+    exx_status st = check_apply_args(p, n_orb, psi_dev, occ_host, kpsi_dev, ex_host);
+    if (st != EXX_OK) return st;
+    if (!is_device_pointer(psi_dev) || !is_device_pointer(kpsi_dev))
+        return fail(p, EXX_ERR_BAD_POINTER, "psi_dev and kpsi_dev must be device pointers");
+    if (is_device_pointer(occ_host) || is_device_pointer(ex_host))
+        return fail(p, EXX_ERR_BAD_POINTER, "occ_host and ex_host must be host pointers");
+    if (psi_dev == kpsi_dev) return fail(p, EXX_ERR_INVALID_ARG, "kpsi must not alias psi");
+    st = apply_impl(p, n_orb, psi_dev, occ_host, kpsi_dev);
+    if (st != EXX_OK) return st;
+    EXX_CUDA(p, cudaMemcpyAsync(p->ex_pinned, p->ex_dev, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    *ex_host = *p->ex_pinned;
+    return EXX_OK;
+}
+
+exx_status exx_apply_host(exx_plan* p, int n_orb, const double* psi_host, const double* occ_host, double* kpsi_host, double* ex_host) {
+    exx_status st = check_apply_args(p, n_orb, psi_host, occ_host, kpsi_host, ex_host);
+    if (st != EXX_OK) return st;
+    if (is_device_pointer(psi_host) || is_device_pointer(kpsi_host) || is_device_pointer(occ_host) || is_device_pointer(ex_host))
+        return fail(p, EXX_ERR_BAD_POINTER, "exx_apply_host takes host pointers");
+    const size_t elems = static_cast<size_t>(n_orb) * p->M;
+    if (elems > p->stage_elems) {
+        if (p->psi_stage) cudaFree(p->psi_stage);
+        if (p->kpsi_stage) cudaFree(p->kpsi_stage);
+        p->psi_stage = p->kpsi_stage = nullptr;
+        p->stage_elems = 0;
+        if (cudaMalloc(&p->psi_stage, elems * sizeof(double)) != cudaSuccess || cudaMalloc(&p->kpsi_stage, elems * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(p, EXX_ERR_ALLOC, "cudaMalloc(host staging) failed");
+        }
+        p->stage_elems = elems;
+    }
+    EXX_CUDA(p, cudaMemcpyAsync(p->psi_stage, psi_host, elems * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    st = apply_impl(p, n_orb, p->psi_stage, occ_host, p->kpsi_stage);
+    if (st != EXX_OK) return st;
+    EXX_CUDA(p, cudaMemcpyAsync(kpsi_host, p->kpsi_stage, elems * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    EXX_CUDA(p, cudaMemcpyAsync(p->ex_pinned, p->ex_dev, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    *ex_host = *p->ex_pinned;
+    return EXX_OK;
+}
+
+exx_status exx_get_pair_energies(exx_plan* p, double* e_host) {
+    if (!p || !e_host) return EXX_ERR_INVALID_ARG;
+    if (p->last_n_orb < 1) return fail(p, EXX_ERR_INVALID_ARG, "no apply has run on this plan");
+    const size_t n = static_cast<size_t>(p->last_n_orb);
+    EXX_CUDA(p, cudaMemcpyAsync(e_host, p->e_mat, n * n * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    return EXX_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,89 @@
+"""Host-side logic of the CUDA library that needs no GPU: exported symbols, scheduler counts, argument checks."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1712_07973_b200 as exx
+from paper_1712_07973_b200.binding import EXPORTS
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLDEN = os.path.join(ROOT, "tests", "golden")
+
+
+def test_library_loads_and_exports_every_declared_symbol():
+    lib = exx.load_library()
+    header = open(os.path.join(ROOT, "include", "exx.h")).read()
+    declared = set(re.findall(r"\b(exx_[a-z_]+)\s*\(", header))
+    declared -= {"exx_plan", "exx_status", "exx_bc"}
+    assert declared, "no declarations found in include/exx.h"
+    for name in sorted(declared):
+        assert hasattr(lib, name), f"{name} declared in include/exx.h but not exported"
+    assert declared == set(EXPORTS), "binding.EXPORTS out of sync with include/exx.h"
+    assert "sm_100a" in exx.exx_version()
+
+
+def test_p10_pair_counts_match_table1():
+    """Scheduler count = N(N+1)/2 = PAPER.md:179-185 Table 1 (H2O columns)."""
+    rows = [line.split() for line in open(os.path.join(GOLDEN, "table1_pair_counts.txt")) if line[0].isdigit()]
+    assert len(rows) == 4
+    for n_orb, solves in rows:
+        n_orb, solves = int(n_orb), int(solves)
+        n_pairs, n_x = exx.exx_schedule_pairs([2.0] * n_orb)
+        assert n_pairs == solves == n_orb * (n_orb + 1) // 2
+        # rows with an odd number of pairs end with a half-empty transform
+        assert n_x == sum((n_orb - i + 1) // 2 for i in range(n_orb))
+
+
+def test_scheduler_skips_only_doubly_empty_pairs():
+    occ = [2.0, 0.0, 1.0, 0.0, 0.0]
+    n_pairs, n_x = exx.exx_schedule_pairs(occ)
+    expect = sum(1 for i in range(5) for j in range(i, 5) if not (occ[i] == 0 and occ[j] == 0))
+    assert n_pairs == expect == 9
+    assert exx.exx_schedule_pairs([0.0, 0.0]) == (0, 0)
+    assert exx.exx_schedule_pairs([1.0]) == (1, 1)
+
+
+def test_status_codes_without_compute():
+    lib = exx.load_library()
+    assert lib.exx_status_string(0) == b"EXX_OK"
+    assert lib.exx_status_string(2) == b"EXX_ERR_UNSUPPORTED_SIZE"
+    h = C.c_void_p()
+    d = (C.c_int * 3)(30, 32, 32)          # 30 = 2*3*5: not a supported length
+    sp = (C.c_double * 3)(0.4, 0.4, 0.4)
+    assert lib.exx_plan_create(C.byref(h), d, sp, 0, None, 4, None) == 2
+    assert b"transform lengths" in lib.exx_last_error(None)
+    d = (C.c_int * 3)(32, 32, 32)
+    assert lib.exx_plan_create(C.byref(h), d, sp, 7, None, 4, None) == 1          # bad enum
+    assert lib.exx_plan_create(C.byref(h), d, sp, 1, None, 4, None) == 1          # free BC without a table
+    sp_bad = (C.c_double * 3)(0.4, -1.0, 0.4)
+    assert lib.exx_plan_create(C.byref(h), d, sp_bad, 0, None, 4, None) == 1
+    assert lib.exx_plan_create(C.byref(h), d, sp, 0, None, 0, None) == 1          # max_orbitals < 1
+    d = (C.c_int * 3)(32, 64, 96)                                                 # mixed lengths only up to 64
+    assert lib.exx_plan_create(C.byref(h), d, sp, 0, None, 4, None) == 2
+    assert lib.exx_plan_destroy(None) == 0
+    assert lib.exx_plan_workspace_bytes(None) == 0
+
+
+def test_no_cpu_fallback():
+    """Without a GPU the product path fails loudly (EXX_ERR_CUDA); with one it must succeed.  Never a CPU result."""
+    import torch
+    if torch.cuda.is_available():
+        plan = exx.ExxPlan((16, 16, 16), (0.4, 0.4, 0.4), "periodic", max_orbitals=2)
+        plan.destroy()
+    else:
+        with pytest.raises(exx.ExxError) as ei:
+            exx.ExxPlan((16, 16, 16), (0.4, 0.4, 0.4), "periodic", max_orbitals=2)
+        assert ei.value.status_name == "EXX_ERR_CUDA"
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1712_07973_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".hpp", ".cpp")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, re.M), f
+                assert "exx_oracle" not in src, f
