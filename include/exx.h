@@ -107,6 +107,14 @@ size_t     exx_plan_workspace_bytes(const exx_plan *plan);
 /* Number of kernel launches the library has enqueued for this plan since creation (for bench "gpu_launches"). */
 long long  exx_plan_launch_count(const exx_plan *plan);
 
+/*
+ * Per-pass device timing (CUDA events on the plan's stream around every pass launch).  Off by default.
+ * exx_plan_get_profile synchronises and returns, for the most recent apply, the summed milliseconds and the
+ * launch counts of  [0] pass A, [1] pass B, [2] pass C, [3] energy reduction.
+ */
+exx_status exx_plan_set_profiling(exx_plan *plan, int enable);
+exx_status exx_plan_get_profile(exx_plan *plan, double pass_ms[4], long long pass_launches[4]);
+
 /* Tuning knob: maximum packed transforms per batch (same-i group); <= 0 restores the default. */
 exx_status exx_plan_set_batch(exx_plan *plan, int max_transforms_per_batch);
 

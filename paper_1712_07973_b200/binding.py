@@ -23,7 +23,7 @@ _STATUS = ["EXX_OK", "EXX_ERR_INVALID_ARG", "EXX_ERR_UNSUPPORTED_SIZE", "EXX_ERR
 EXPORTS = [
     "exx_plan_create", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_get_pair_energies",
     "exx_schedule_pairs", "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count",
-    "exx_plan_set_batch", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version",
+    "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version",
 ]
 
 _lib = None
@@ -68,6 +68,10 @@ def load_library():
     lib.exx_plan_launch_count.restype = C.c_longlong
     lib.exx_plan_set_batch.argtypes = [C.c_void_p, C.c_int]
     lib.exx_plan_set_batch.restype = C.c_int
+    lib.exx_plan_set_profiling.argtypes = [C.c_void_p, C.c_int]
+    lib.exx_plan_set_profiling.restype = C.c_int
+    lib.exx_plan_get_profile.argtypes = [C.c_void_p, _dp, C.POINTER(C.c_longlong)]
+    lib.exx_plan_get_profile.restype = C.c_int
     lib.exx_plan_destroy.argtypes = [C.c_void_p]
     lib.exx_plan_destroy.restype = C.c_int
     lib.exx_status_string.argtypes = [C.c_int]
@@ -139,6 +143,16 @@ class ExxPlan:
 
     def set_batch(self, n: int):
         self._check(load_library().exx_plan_set_batch(self._h, int(n)))
+
+    def set_profiling(self, enable: bool):
+        self._check(load_library().exx_plan_set_profiling(self._h, 1 if enable else 0))
+
+    def get_profile(self):
+        """Per-pass (A, B, C, reduce) summed device milliseconds and launch counts of the most recent apply."""
+        ms = (C.c_double * 4)()
+        n = (C.c_longlong * 4)()
+        self._check(load_library().exx_plan_get_profile(self._h, ms, n))
+        return list(ms), list(n)
 
     # -- the hot path
     def apply(self, psi, occ, kpsi=None):

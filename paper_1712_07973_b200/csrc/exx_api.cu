@@ -158,6 +158,9 @@ struct exx_plan {
     KernelInfo info_ac, info_b;
     long long launches;
     int last_n_orb;
+    int profiling;
+    std::vector<cudaEvent_t> events;   // 5 per batch when profiling
+    size_t events_used;
     size_t ws_bytes;        // batch workspace (W1 + energy partials)
     size_t fixed_bytes;     // tables, descriptors, pair-energy matrix
     std::string err;
@@ -329,14 +332,32 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
     split_of(p->t[2], &ab.pc, &ab.qc);
     ab.npch = p->t[2] >> p->geo.chunk_log2;
 
+    p->events_used = 0;
+    if (p->profiling) {
+        const size_t need = sched.batches.size() * 5;
+        while (p->events.size() < need) {
+            cudaEvent_t ev;
+            EXX_CUDA(p, cudaEventCreate(&ev));
+            p->events.push_back(ev);
+        }
+    }
+    auto mark = [&]() -> cudaError_t {
+        if (!p->profiling) return cudaSuccess;
+        return cudaEventRecord(p->events[p->events_used++], s);
+    };
     for (const Batch& b : sched.batches) {
         ac.desc = p->desc_dev + b.first;
         ac.i = b.i; ac.fi = occ_host[b.i]; ac.count = b.count;
+        EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_a(p->geo, ac, b.count, s, nullptr));
+        EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_b(p->geo, ab, b.count, s, nullptr));
+        EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
+        EXX_CUDA(p, mark());
         reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_ac.tiles, ac.desc, b.i, n_orb, p->dV, p->e_mat);
         EXX_CUDA(p, cudaGetLastError());
+        EXX_CUDA(p, mark());
         p->launches += 4;
     }
     exchange_energy_kernel<<<1, 1024, 0, s>>>(p->e_mat, p->occ_dev, n_orb, p->ex_dev);
@@ -505,6 +526,7 @@ exx_status exx_plan_destroy(exx_plan* p) {
     if (p->occ_pinned) cudaFreeHost(p->occ_pinned);
     if (p->ex_pinned) cudaFreeHost(p->ex_pinned);
     if (p->upload_done) cudaEventDestroy(p->upload_done);
+    for (cudaEvent_t ev : p->events) cudaEventDestroy(ev);
     if (p->psi_stage) cudaFree(p->psi_stage);
     if (p->kpsi_stage) cudaFree(p->kpsi_stage);
     cudaGetLastError();
@@ -521,6 +543,29 @@ exx_status exx_plan_transform_dims(const exx_plan* p, int tdims[3]) {
 size_t exx_plan_workspace_bytes(const exx_plan* p) { return p ? p->ws_bytes + p->fixed_bytes : 0; }
 
 long long exx_plan_launch_count(const exx_plan* p) { return p ? p->launches : 0; }
+
+exx_status exx_plan_set_profiling(exx_plan* p, int enable) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    p->profiling = enable ? 1 : 0;
+    p->events_used = 0;
+    return EXX_OK;
+}
+
+exx_status exx_plan_get_profile(exx_plan* p, double pass_ms[4], long long pass_launches[4]) {
+    if (!p || !pass_ms || !pass_launches) return EXX_ERR_INVALID_ARG;
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    for (int k = 0; k < 4; ++k) { pass_ms[k] = 0.0; pass_launches[k] = 0; }
+    for (size_t b = 0; b + 5 <= p->events_used; b += 5) {
+        for (int k = 0; k < 4; ++k) {
+            float ms = 0.f;
+            EXX_CUDA(p, cudaEventElapsedTime(&ms, p->events[b + k], p->events[b + k + 1]));
+            pass_ms[k] += ms;
+            pass_launches[k] += 1;
+        }
+    }
+    return EXX_OK;
+}
 
 exx_status exx_plan_set_batch(exx_plan* p, int max_transforms_per_batch) {
     if (!p) return EXX_ERR_INVALID_ARG;
