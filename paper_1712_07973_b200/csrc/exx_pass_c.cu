@@ -8,16 +8,18 @@ template <int TC, int TB, bool FREE>
 static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
     using T = TuneAC<TC, TB, FREE>;
     using C = typename T::Cfg;
-    constexpr int smem = C::SMEM_ELEMS * static_cast<int>(sizeof(double2));
-    auto kern = pass_c_kernel<C, T::NT>;
-    if (info) { info->threads = T::NT; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; }
+    constexpr int NSTG = T::NSTG_C;                          // operand stages (psi_j, psi_l lines in flight)
+    constexpr int smem = T::SMEM_C;
+    static_assert(smem == (2 * C::SMEM_C * 16 + NSTG * C::OP_DOUBLES * 8) && smem <= kMaxSmemC, "pass C shared memory");
+    auto kern = pass_c_kernel<C, T::NT_C, NSTG>;
+    if (info) { info->threads = T::NT_C; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; }
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    kern<<<args.na * C::TILES_PER_A, T::NT, smem, s>>>(args);
+    kern<<<args.na * C::TILES_PER_A, T::NT_C, smem, s>>>(args);
     return cudaGetLastError();
 }
 

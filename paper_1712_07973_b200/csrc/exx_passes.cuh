@@ -28,6 +28,7 @@
 
 #include <cuda_runtime.h>
 
+#include "exx_async.cuh"
 #include "exx_dft.cuh"
 
 namespace exx {
@@ -111,6 +112,17 @@ struct CfgAC {
     static constexpr int ITEMS_POS = G * TC;               // (g, position) items: phases A2, C0
     static_assert(R2 % G == 0, "G must divide R2");
     EXX_HD static int spos(int p) { return (p / QC) * QCP + (p % QC); }
+    // ---- pass C (v2): the W1 tile lands in place in the work buffer, which therefore has R1 lines per b2 of the tile
+    static constexpr int GPAD = G > 1 ? 4 : 0;             // shifts consecutive b2 groups by 64 B (bank conflicts)
+    static constexpr int GSTR_C = R1 * ROW + GPAD;         // elements between the line blocks of consecutive gi
+    static constexpr int SMEM_C = G * GSTR_C;              // elements of one pass-C work buffer
+    static constexpr int TILE_ELEMS = G * R1 * TC;         // complex values of one W1 tile
+    // operand lines (psi_j, psi_l; overwritten with the K psi_j, K psi_l increments) staged in shared memory:
+    // line stride LS doubles, LS = QC (mod 16) keeps the (line, n2)-mapped 8-byte accesses conflict-free
+    static constexpr int LS = NC + (((QC - NC % 16) % 16) + 16) % 16;
+    static constexpr int OP_DOUBLES = 2 * LINES * LS;      // one stage: [slot j|l][line][LS]
+    static_assert(LS % 2 == 0 && NC % 2 == 0, "16-byte alignment of operand lines");
+    EXX_HD static int line_c(int gi, int q) { return gi * GSTR_C + q * ROW; }
 };
 
 struct ArgsAC {
@@ -193,23 +205,36 @@ EXX_HD void a2_item(int w, const double2* S, const ArgsAC& g, int t, int a, int 
     }
 }
 
-// ---- C0: load from W1, conj twiddle, inverse R1 stage of the b axis
+// ---- C landing: element e of the W1 tile of (t, a, b2base) -> (index in W1, element offset in the work buffer).
+//      e enumerates (q, pch, gi, pin) with pin fastest, then gi: consecutive e are consecutive in W1 for G*CHUNK
+//      elements (128 B runs for G*CHUNK = 8), so a warp's 16-byte cp.async requests coalesce into full lines.
 template <class C>
-EXX_HD void c0_item(int w, double2* S, const ArgsAC& g, int t, int a, int b2base) {
+EXX_HD void c_land_map(int e, const ArgsAC& g, int t, int a, int b2base, size_t* src, int* dst) {
+    const int chunk = 1 << g.chunk_log2;
+    const int npch = C::TC >> g.chunk_log2;
+    const int pin = e & (chunk - 1);
+    int r = e >> g.chunk_log2;
+    const int gi = r % C::G; r /= C::G;
+    const int pch = r % npch;
+    const int q = r / npch;
+    *src = w1_index<C::R1, C::R2>(t, q, pch, a, b2base + gi, pin, npch, g.na, chunk);
+    *dst = C::line_c(gi, q) + C::spos(pch * chunk + pin);
+}
+
+// ---- C0: conj twiddle + inverse R1 stage of the b axis, in place in the work buffer (q lines -> b1 lines)
+template <class C>
+EXX_HD void c0_item(int w, double2* S, const ArgsAC& g, int b2base) {
     const int gi = w / C::TC, p = w % C::TC;
     const int b2 = b2base + gi;
-    const int chunk = 1 << g.chunk_log2;
-    const int pch = p >> g.chunk_log2, pin = p & (chunk - 1);
-    const int npch = C::TC >> g.chunk_log2;
+    double2* col = S + C::line_c(gi, 0) + C::spos(p);
     double xr[C::R1], xi[C::R1];
 #pragma unroll
     for (int q = 0; q < C::R1; ++q) {
-        double2 v = g.w1[w1_index<C::R1, C::R2>(t, q, pch, a, b2, pin, npch, g.na, chunk)];
+        double2 v = col[q * C::ROW];
         xr[q] = v.x; xi[q] = v.y;
         if (q > 0) cmul_conj(xr[q], xi[q], ld_ro(g.rootsb + (b2 * q) % C::TB));
     }
     dft_inv<C::R1, C::FREE>(xr, xi);
-    double2* col = S + gi * C::NB1 * C::ROW + C::spos(p);
 #pragma unroll
     for (int b1 = 0; b1 < C::NB1; ++b1) col[b1 * C::ROW] = make_double2(xr[b1], xi[b1]);
 }
@@ -218,7 +243,7 @@ EXX_HD void c0_item(int w, double2* S, const ArgsAC& g, int t, int a, int b2base
 template <class C>
 EXX_HD void c1_item(int w, double2* S, const ArgsAC& g) {
     const int l = w / C::PC, k1 = w % C::PC;
-    double2* seg = S + l * C::ROW + k1 * C::QCP;
+    double2* seg = S + C::line_c(l / C::NB1, l % C::NB1) + k1 * C::QCP;
     double xr[C::QC], xi[C::QC];
 #pragma unroll
     for (int k2 = 0; k2 < C::QC; ++k2) { double2 v = seg[k2]; xr[k2] = v.x; xi[k2] = v.y; }
@@ -230,45 +255,36 @@ EXX_HD void c1_item(int w, double2* S, const ArgsAC& g) {
     }
 }
 
-// ---- C2: inverse stage over k1 (P-point) of the c axis, then "Kernel 3":
+// ---- C2: inverse stage over k1 (P-point) of the c axis, then "Kernel 3" for the PCN points
+//      c = QC n1 + n2 of line l that this item owns:
 //      acc   += f_j V_ij psi_j + f_l V_il psi_l                 (K psi_i -= acc after the batch)
-//      Kpsi_j -= f_i V_ij psi_i   (j != i),   Kpsi_l -= f_i V_il psi_i   (l != i)     PAPER.md:67-69 Eq. 3, :111
+//      oj    <- -f_i V_ij psi_i ,  ol <- -f_i V_il psi_i         increments of K psi_j, K psi_l, written over the
+//               staged psi_j / psi_l values and added to K psi by the memory system   PAPER.md:67-69 Eq. 3, :111
 //      e1    += rho_ij V_ij,  e2 += rho_il V_il                                        PAPER.md:81-82 Eq. 5
+//      vi = psi_i at the item's points; oj / ol = operand lines of this item at offset n2 (stride QC between n1).
 template <class C>
-EXX_HD void c2_item(int w, const double2* S, const ArgsAC& g, const XformDesc& d, int a, int b2base,
-                    double* acc /*[PCN]*/, double& e1, double& e2) {
+EXX_HD void c2_item(int w, const double2* S, const XformDesc& d, double fi, const double* vi /*[PCN]*/, double* oj,
+                    double* ol, double* acc /*[PCN]*/, double& e1, double& e2) {
     const int l = w / C::QC, n2 = w % C::QC;
-    const int gi = l / C::NB1, b1 = l % C::NB1;
-    const int b = C::R2 * b1 + b2base + gi;
-    const double2* row = S + l * C::ROW + n2;
+    const double2* row = S + C::line_c(l / C::NB1, l % C::NB1) + n2;
     double xr[C::PC], xi[C::PC];
 #pragma unroll
     for (int k1 = 0; k1 < C::PC; ++k1) { double2 v = row[k1 * C::QCP]; xr[k1] = v.x; xi[k1] = v.y; }
     dft_inv<C::PC, C::FREE>(xr, xi);
-    const size_t base = (static_cast<size_t>(a) * C::NB + b) * C::NC + n2;
-    const double* pi = g.psi + static_cast<size_t>(g.i) * g.m_points + base;
-    const double* pj = g.psi + static_cast<size_t>(d.j) * g.m_points + base;
-    double* kj = g.kpsi + static_cast<size_t>(d.j) * g.m_points + base;
     const bool has_l = d.l >= 0;
-    const int lidx = has_l ? d.l : d.j;
-    const double* pl = g.psi + static_cast<size_t>(lidx) * g.m_points + base;
-    double* kl = g.kpsi + static_cast<size_t>(lidx) * g.m_points + base;
-    const bool upd_j = d.j != g.i;
-    const bool upd_l = has_l && d.l != g.i;
     const double fl = has_l ? d.fl : 0.0;
     double s1 = 0.0, s2 = 0.0;
 #pragma unroll
     for (int n1 = 0; n1 < C::PCN; ++n1) {
         const int off = C::QC * n1;
         const double v1 = xr[n1], v2 = xi[n1];
-        const double vi = ld_ro(pi + off);
-        const double vj = ld_ro(pj + off);
-        const double vl = has_l ? ld_ro(pl + off) : 0.0;
+        const double vj = oj[off];
+        const double vl = has_l ? ol[off] : 0.0;
         acc[n1] += d.fj * v1 * vj + fl * v2 * vl;
-        if (upd_j) kj[off] -= g.fi * v1 * vi;
-        if (upd_l) kl[off] -= g.fi * v2 * vi;
-        s1 += vi * vj * v1;
-        s2 += vi * vl * v2;
+        oj[off] = -(fi * v1 * vi[n1]);
+        if (has_l) ol[off] = -(fi * v2 * vi[n1]);
+        s1 += vi[n1] * vj * v1;
+        s2 += vi[n1] * vl * v2;
     }
     e1 += s1;
     e2 += s2;
@@ -425,27 +441,95 @@ __global__ void __launch_bounds__(NT) pass_b_kernel(const ArgsB g) {
     for (int w = threadIdx.x; w < C::ITEMS_IO; w += NT) b4_item<C>(w, S, g, t, q, pch);
 }
 
-// One CTA per (a, b2-group) tile; loops over the transforms of the same-i batch and keeps the K psi_i
-// accumulator of its tile in registers.  NT >= ITEMS_LINE_Q (one epilogue item per thread).
-template <class C, int NT>
-__global__ void __launch_bounds__(NT) pass_c_kernel(const ArgsAC g) {
+// Pass C.  One CTA per (a, b2-group) tile; it loops over the transforms of the same-i batch, keeps the K psi_i
+// accumulator and psi_i of its points in registers, and is software-pipelined:
+//   * the W1 tile of transform t+1 is gathered into the second work buffer with 16-byte cp.async while t is computed;
+//   * psi_j / psi_l lines arrive NSTG transforms ahead by TMA bulk copies (mbarrier completion) into operand stages;
+//   * the K psi_j / K psi_l increments overwrite those lines and leave by TMA bulk reduce-add (fp64) -- each K psi
+//     address receives exactly one add per launch (the j of a batch are distinct), so the result is deterministic.
+// NT >= ITEMS_LINE_Q (one epilogue item per thread).
+template <class C, int NT, int NSTG>
+__global__ void __launch_bounds__(NT, 1) pass_c_kernel(const ArgsAC g) {
     static_assert(NT >= C::ITEMS_LINE_Q, "pass C needs one thread per epilogue item");
-    extern __shared__ double2 S[];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* const S0 = reinterpret_cast<double2*>(smem_raw);
+    double* const OP = reinterpret_cast<double*>(S0 + 2 * C::SMEM_C);
+    __shared__ uint64_t full[NSTG];
     __shared__ double red[2][NT / 32];
     const int tile = blockIdx.x;
     const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
     const int tid = threadIdx.x;
-    double acc[C::PCN];
-#pragma unroll
-    for (int n1 = 0; n1 < C::PCN; ++n1) acc[n1] = 0.0;
-    for (int t = 0; t < g.count; ++t) {
+    constexpr uint32_t LINE_BYTES = C::NC * sizeof(double);
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    // operand traffic of transform t (warp 0): loads of psi_j / psi_l lines, later reduce-adds of the increments
+    auto line_gmem = [&](int orb, int l) -> size_t {
+        const int gi = l / C::NB1, b1 = l % C::NB1;
+        const int b = C::R2 * b1 + b2base + gi;
+        return static_cast<size_t>(orb) * g.m_points + (static_cast<size_t>(a) * C::NB + b) * C::NC;
+    };
+    auto issue_operand_loads = [&](int t) {          // called by all lanes of warp 0
         const XformDesc d = g.desc[t];
-        for (int w = tid; w < C::ITEMS_POS; w += NT) c0_item<C>(w, S, g, t, a, b2base);
+        const int s = t % NSTG;
+        double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
+        const int nops = (d.l >= 0 ? 2 : 1) * C::LINES;
+        if (tid == 0) mbar_arrive_expect_tx(&full[s], nops * LINE_BYTES);
+        __syncwarp();
+        for (int o = tid; o < nops; o += 32) {
+            const int slot = o / C::LINES, l = o % C::LINES;
+            bulk_g2s(stage + (slot * C::LINES + l) * C::LS, g.psi + line_gmem(slot ? d.l : d.j, l), LINE_BYTES, &full[s]);
+        }
+    };
+    auto issue_w1_gather = [&](int t) {              // all threads
+        double2* dstbuf = S0 + (t & 1) * C::SMEM_C;
+        for (int e = tid; e < C::TILE_ELEMS; e += NT) {
+            size_t src; int dst;
+            c_land_map<C>(e, g, t, a, b2base, &src, &dst);
+            cp_async16(dstbuf + dst, g.w1 + src);
+        }
+    };
+
+    issue_w1_gather(0);
+    cp_async_commit();
+    if (tid < 32)
+        for (int t = 0; t < NSTG && t < g.count; ++t) issue_operand_loads(t);
+
+    // this thread's epilogue item: PCN points of one line
+    const int my_l = tid / C::QC, my_n2 = tid % C::QC;
+    double vi[C::PCN], acc[C::PCN];
+#pragma unroll
+    for (int n1 = 0; n1 < C::PCN; ++n1) { vi[n1] = 0.0; acc[n1] = 0.0; }
+    if (tid < C::ITEMS_LINE_Q) {
+        const double* pi = g.psi + line_gmem(g.i, my_l) + my_n2;
+#pragma unroll
+        for (int n1 = 0; n1 < C::PCN; ++n1) vi[n1] = ld_ro(pi + C::QC * n1);
+    }
+
+    for (int t = 0; t < g.count; ++t) {
+        double2* S = S0 + (t & 1) * C::SMEM_C;
+        const int s = t % NSTG;
+        double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
+        const XformDesc d = g.desc[t];
+        if (t + 1 < g.count) issue_w1_gather(t + 1);
+        cp_async_commit();
+        cp_async_wait<1>();                                // this thread's part of tile t has landed
+        __syncthreads();
+        for (int w = tid; w < C::ITEMS_POS; w += NT) c0_item<C>(w, S, g, b2base);
         __syncthreads();
         for (int w = tid; w < C::ITEMS_LINE_P; w += NT) c1_item<C>(w, S, g);
         __syncthreads();
+        mbar_wait(&full[s], (t / NSTG) & 1);               // psi_j / psi_l lines of transform t have landed
         double e1 = 0.0, e2 = 0.0;
-        if (tid < C::ITEMS_LINE_Q) c2_item<C>(tid, S, g, d, a, b2base, acc, e1, e2);
+        if (tid < C::ITEMS_LINE_Q) {
+            double* oj = stage + my_l * C::LS + my_n2;
+            c2_item<C>(tid, S, d, g.fi, vi, oj, oj + C::LINES * C::LS, acc, e1, e2);
+        }
+        fence_proxy_async();                               // increments visible to the TMA reads below
         // block reduction of the energy partials in a fixed order (deterministic)
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -453,7 +537,7 @@ __global__ void __launch_bounds__(NT) pass_c_kernel(const ArgsAC g) {
             e2 += __shfl_xor_sync(0xffffffffu, e2, o);
         }
         if ((tid & 31) == 0) { red[0][tid >> 5] = e1; red[1][tid >> 5] = e2; }
-        __syncthreads();                                   // also protects S before the next transform
+        __syncthreads();                                   // also: S and the operand stage are no longer read
         if (tid == 0) {
             double s1 = 0.0, s2 = 0.0;
 #pragma unroll
@@ -461,8 +545,24 @@ __global__ void __launch_bounds__(NT) pass_c_kernel(const ArgsAC g) {
             double* ep = g.epart + (static_cast<size_t>(t) * gridDim.x + tile) * 2;
             ep[0] = s1; ep[1] = s2;
         }
+        if (tid < 32) {
+            // K psi_j += -f_i V_ij psi_i,  K psi_l += -f_i V_il psi_i   (the same V_ij serves both orbitals)
+            const bool upd_j = d.j != g.i, upd_l = d.l >= 0 && d.l != g.i;
+            for (int o = tid; o < 2 * C::LINES; o += 32) {
+                const int slot = o / C::LINES, l = o % C::LINES;
+                if (slot ? upd_l : upd_j)
+                    bulk_red_add_f64(g.kpsi + line_gmem(slot ? d.l : d.j, l), stage + (slot * C::LINES + l) * C::LS, LINE_BYTES);
+            }
+            bulk_commit();
+            if (t + NSTG < g.count) {
+                bulk_wait_read_all();                      // the stage may be overwritten
+                __syncwarp();
+                issue_operand_loads(t + NSTG);
+            }
+        }
     }
     if (tid < C::ITEMS_LINE_Q) c_flush_item<C>(tid, g, a, b2base, acc);
+    if (tid < 32) bulk_wait_read_all();                    // shared memory must outlive the TMA reads
 }
 
 #endif  // __CUDACC__

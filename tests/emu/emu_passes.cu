@@ -47,19 +47,49 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
             for (int w = 0; w < B::ITEMS_Q; ++w) b3_item<B>(w, S.data());
             for (int w = 0; w < B::ITEMS_IO; ++w) b4_item<B>(w, S.data(), gb, t, q, pch);
         }
-    // pass C
-    std::vector<double> acc(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN);
+    // pass C (v2): W1 tile landed in place in the work buffer (c_land_map = the kernel's cp.async gather), psi_j / psi_l
+    // lines staged in an operand buffer that c2 overwrites with the K psi_j / K psi_l increments (the kernel's TMA
+    // bulk loads and bulk reduce-adds are plain copies / adds here).
+    std::vector<double2> SC(AC::SMEM_C);
+    std::vector<double> op(AC::OP_DOUBLES);
+    std::vector<double> acc(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN), vi(acc.size());
+    auto line_gmem = [&](int orb, int l, int a, int b2base) {
+        const int gi = l / AC::NB1, b1 = l % AC::NB1;
+        const int b = AC::R2 * b1 + b2base + gi;
+        return static_cast<size_t>(orb) * m_points + (static_cast<size_t>(a) * AC::NB + b) * AC::NC;
+    };
     for (int tile = 0; tile < ntiles; ++tile) {
         const int a = tile / AC::TILES_PER_A, b2base = (tile % AC::TILES_PER_A) * G;
         std::fill(acc.begin(), acc.end(), 0.0);
+        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w)
+            for (int n1 = 0; n1 < AC::PCN; ++n1)
+                vi[static_cast<size_t>(w) * AC::PCN + n1] = psi[line_gmem(i, w / AC::QC, a, b2base) + w % AC::QC + AC::QC * n1];
         for (int t = 0; t < count; ++t) {
-            for (int w = 0; w < AC::ITEMS_POS; ++w) c0_item<AC>(w, S.data(), g, t, a, b2base);
-            for (int w = 0; w < AC::ITEMS_LINE_P; ++w) c1_item<AC>(w, S.data(), g);
+            for (int e = 0; e < AC::TILE_ELEMS; ++e) {
+                size_t src; int dst;
+                c_land_map<AC>(e, g, t, a, b2base, &src, &dst);
+                SC[dst] = w1[src];
+            }
+            for (int w = 0; w < AC::ITEMS_POS; ++w) c0_item<AC>(w, SC.data(), g, b2base);
+            for (int w = 0; w < AC::ITEMS_LINE_P; ++w) c1_item<AC>(w, SC.data(), g);
+            const XformDesc d = desc[t];
+            for (int slot = 0; slot < (d.l >= 0 ? 2 : 1); ++slot)
+                for (int l = 0; l < AC::LINES; ++l)
+                    std::memcpy(&op[(slot * AC::LINES + l) * AC::LS], psi + line_gmem(slot ? d.l : d.j, l, a, b2base), AC::NC * sizeof(double));
             double e1 = 0.0, e2 = 0.0;
-            for (int w = 0; w < AC::ITEMS_LINE_Q; ++w)
-                c2_item<AC>(w, S.data(), g, desc[t], a, b2base, acc.data() + static_cast<size_t>(w) * AC::PCN, e1, e2);
+            for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
+                double* oj = &op[(w / AC::QC) * AC::LS + w % AC::QC];
+                c2_item<AC>(w, SC.data(), d, fi, &vi[static_cast<size_t>(w) * AC::PCN], oj, oj + AC::LINES * AC::LS,
+                            &acc[static_cast<size_t>(w) * AC::PCN], e1, e2);
+            }
             e_out[2 * t] += e1;
             e_out[2 * t + 1] += e2;
+            for (int slot = 0; slot < 2; ++slot) {
+                const int orb = slot ? d.l : d.j;
+                if (orb < 0 || orb == i) continue;
+                for (int l = 0; l < AC::LINES; ++l)
+                    for (int c = 0; c < AC::NC; ++c) kpsi[line_gmem(orb, l, a, b2base) + c] += op[(slot * AC::LINES + l) * AC::LS + c];
+            }
         }
         for (int w = 0; w < AC::ITEMS_LINE_Q; ++w)
             c_flush_item<AC>(w, g, a, b2base, acc.data() + static_cast<size_t>(w) * AC::PCN);
