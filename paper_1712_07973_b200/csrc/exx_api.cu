@@ -79,6 +79,21 @@ __global__ void cos_transform_kernel(const double* in, double* out, long long ou
     }
 }
 
+// ks_perm[sa][sb][p] = ks_sym[sa][sb][sc(p)]: the c index in the digit-scrambled order of the in-tile FFT
+// (position p = k1*QC + k2 holds frequency kc = k1 + PC*k2), so that pass B reads K^ contiguously along pin.
+__global__ void permute_kernel_c_axis(const double* ks_sym, double* ks_perm, long long rows, int tc, int pc, int qc) {
+    const int nch = tc / 2 + 1;
+    const long long total = rows * tc;
+    for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
+         x += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int p = static_cast<int>(x % tc);
+        const long long row = x / tc;
+        const int kc = (p / qc) + pc * (p % qc);
+        const int sc = kc <= tc - kc ? kc : tc - kc;
+        ks_perm[x] = ks_sym[row * nch + sc];
+    }
+}
+
 // e_ij = dV * sum over tiles of the per-CTA partial sums of pass C, fixed order (deterministic).
 __global__ void reduce_energy_kernel(const double* epart, int tiles, const XformDesc* desc, int i, int n_orb, double dV,
                                      double* e_mat) {
@@ -139,7 +154,8 @@ struct exx_plan {
     cudaStream_t stream;
     double2* tw[3];
     double2* roots[3];
-    double* ks;
+    double2* twb;           // [b2*R1 + q] = W_TB^{b2 q}
+    double* ks;             // [TA/2+1][TB/2+1][TC], c index in scrambled order
     double2* w1;
     size_t w1_elems_per_xform;
     double* epart;
@@ -155,7 +171,7 @@ struct exx_plan {
     double* psi_stage;
     double* kpsi_stage;
     size_t stage_elems;
-    KernelInfo info_ac, info_b;
+    KernelInfo info_a, info_b, info_c;
     long long launches;
     int last_n_orb;
     int profiling;
@@ -229,6 +245,18 @@ void split_of(int T, int* P, int* Q) {
     }
 }
 
+void bsplit_of(int T, int* R1, int* R2) {
+    switch (T) {
+        case 16: *R1 = BSplit<16>::R1; *R2 = BSplit<16>::R2; break;
+        case 32: *R1 = BSplit<32>::R1; *R2 = BSplit<32>::R2; break;
+        case 64: *R1 = BSplit<64>::R1; *R2 = BSplit<64>::R2; break;
+        case 96: *R1 = BSplit<96>::R1; *R2 = BSplit<96>::R2; break;
+        case 128: *R1 = BSplit<128>::R1; *R2 = BSplit<128>::R2; break;
+        case 192: *R1 = BSplit<192>::R1; *R2 = BSplit<192>::R2; break;
+        default: *R1 = BSplit<256>::R1; *R2 = BSplit<256>::R2; break;
+    }
+}
+
 void free_workspace(exx_plan* p) {
     if (p->w1) cudaFree(p->w1);
     if (p->epart) cudaFree(p->epart);
@@ -240,7 +268,7 @@ exx_status alloc_workspace(exx_plan* p, int max_batch) {
     free_workspace(p);
     p->max_batch = max_batch;
     const size_t w1_bytes = p->w1_elems_per_xform * sizeof(double2) * static_cast<size_t>(max_batch);
-    const size_t ep_bytes = static_cast<size_t>(max_batch) * p->info_ac.tiles * 2 * sizeof(double);
+    const size_t ep_bytes = static_cast<size_t>(max_batch) * p->info_c.tiles * 2 * sizeof(double);
     cudaError_t e = cudaMalloc(&p->w1, w1_bytes);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(p, EXX_ERR_ALLOC, "cudaMalloc(workspace W1) failed"); }
     e = cudaMalloc(&p->epart, ep_bytes);
@@ -260,20 +288,32 @@ int default_batch(const exx_plan* p) {
 exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
     const int na = p->t[0] / 2 + 1, nb = p->t[1] / 2 + 1, nc = p->t[2] / 2 + 1;
     const size_t total = static_cast<size_t>(na) * nb * nc;
-    if (cudaMalloc(&p->ks, total * sizeof(double)) != cudaSuccess) {
+    const size_t total_perm = static_cast<size_t>(na) * nb * p->t[2];
+    double* ks_sym = nullptr;
+    if (cudaMalloc(&p->ks, total_perm * sizeof(double)) != cudaSuccess || cudaMalloc(&ks_sym, total * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
+        if (ks_sym) cudaFree(ks_sym);
         return fail(p, EXX_ERR_ALLOC, "cudaMalloc(Fourier kernel) failed");
     }
+    struct Guard { double* q; ~Guard() { if (q) cudaFree(q); } } guard{ks_sym};
+    auto permute = [&]() -> cudaError_t {
+        int pc = 0, qc = 0;
+        split_of(p->t[2], &pc, &qc);
+        permute_kernel_c_axis<<<2048, 256, 0, p->stream>>>(ks_sym, p->ks, static_cast<long long>(na) * nb, p->t[2], pc, qc);
+        ++p->launches;
+        cudaError_t e = cudaGetLastError();
+        return e != cudaSuccess ? e : cudaStreamSynchronize(p->stream);
+    };
     const double t_tot = static_cast<double>(p->t[0]) * p->t[1] * p->t[2];
     const int threads = 256;
     if (p->bc == EXX_BC_PERIODIC) {
         const int blocks = static_cast<int>((total + threads - 1) / threads < 4096 ? (total + threads - 1) / threads : 4096);
-        ks_periodic_kernel<<<blocks, threads, 0, p->stream>>>(p->ks, na, nb, nc, 2.0 * kPi / (p->t[0] * p->h[0]),
+        ks_periodic_kernel<<<blocks, threads, 0, p->stream>>>(ks_sym, na, nb, nc, 2.0 * kPi / (p->t[0] * p->h[0]),
                                                               2.0 * kPi / (p->t[1] * p->h[1]),
                                                               2.0 * kPi / (p->t[2] * p->h[2]), 1.0 / t_tot);
         EXX_CUDA(p, cudaGetLastError());
         ++p->launches;
-        EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+        EXX_CUDA(p, permute());
         return EXX_OK;
     }
     // FREE: K^ = dV * DFT3(g_ext) restricted to the symmetric index range, computed as three cosine transforms of
@@ -298,12 +338,12 @@ exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
         cos_transform_kernel<<<blocks_for(t1sz), threads, 0, p->stream>>>(g, t1, 1, n0, na, static_cast<long long>(n1) * n2,
                                                                           p->t[0], 1.0);
         cos_transform_kernel<<<blocks_for(t2sz), threads, 0, p->stream>>>(t1, t2, na, n1, nb, n2, p->t[1], 1.0);
-        cos_transform_kernel<<<blocks_for(total), threads, 0, p->stream>>>(t2, p->ks, static_cast<long long>(na) * nb, n2, nc, 1,
+        cos_transform_kernel<<<blocks_for(total), threads, 0, p->stream>>>(t2, ks_sym, static_cast<long long>(na) * nb, n2, nc, 1,
                                                                            p->t[2], p->dV / t_tot);
         p->launches += 4;
         e = cudaGetLastError();
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    if (e == cudaSuccess) e = permute();
     cudaFree(g); cudaFree(t1); cudaFree(t2);
     if (e != cudaSuccess) return cuda_fail(p, e, "building the free-BC Fourier kernel");
     return EXX_OK;
@@ -325,12 +365,11 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
     EXX_CUDA(p, cudaMemsetAsync(p->e_mat, 0, sizeof(double) * static_cast<size_t>(n_orb) * n_orb, s));
 
     ArgsAC ac{};
-    ac.psi = psi; ac.kpsi = kpsi; ac.w1 = p->w1; ac.twc = p->tw[2]; ac.rootsb = p->roots[1]; ac.epart = p->epart;
-    ac.m_points = p->M; ac.na = p->n[0]; ac.chunk_log2 = p->geo.chunk_log2;
+    ac.psi = psi; ac.kpsi = kpsi; ac.w1 = p->w1; ac.twc = p->tw[2]; ac.twb = p->twb; ac.epart = p->epart;
+    ac.m_points = p->M; ac.na = p->n[0];
     ArgsB ab{};
     ab.w1 = p->w1; ab.twa = p->tw[0]; ab.ks = p->ks; ab.tc = p->t[2];
-    split_of(p->t[2], &ab.pc, &ab.qc);
-    ab.npch = p->t[2] >> p->geo.chunk_log2;
+    ab.npch = p->t[2] / p->geo.chunk;
 
     p->events_used = 0;
     if (p->profiling) {
@@ -349,13 +388,13 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
         ac.desc = p->desc_dev + b.first;
         ac.i = b.i; ac.fi = occ_host[b.i]; ac.count = b.count;
         EXX_CUDA(p, mark());
-        EXX_CUDA(p, launch_pass_a(p->geo, ac, b.count, s, nullptr));
+        EXX_CUDA(p, launch_pass_a(p->geo, ac, s, nullptr));
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_b(p->geo, ab, b.count, s, nullptr));
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
         EXX_CUDA(p, mark());
-        reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_ac.tiles, ac.desc, b.i, n_orb, p->dV, p->e_mat);
+        reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_c.tiles, ac.desc, b.i, n_orb, p->dV, p->e_mat);
         EXX_CUDA(p, cudaGetLastError());
         EXX_CUDA(p, mark());
         p->launches += 4;
@@ -429,7 +468,7 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     if (!geometry_supported(geo))
         return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE,
                     "transform lengths must be in {16,32,64,96,128,192,256}; non-cubic grids only with lengths <= 64");
-    geo.chunk_log2 = default_chunk_log2(geo.ta, geo.tb);
+    geo.chunk = chunk_for(geo.ta, geo.tb, geo.free_bc != 0);
 
     int ndev = 0;
     cudaError_t ce = cudaGetDeviceCount(&ndev);
@@ -461,7 +500,8 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
         exx_plan_destroy(p);
         return st;
     };
-    if (query_pass_ac(geo, &p->info_ac) != cudaSuccess || query_pass_b(geo, &p->info_b) != cudaSuccess)
+    if (query_pass_a(geo, &p->info_a) != cudaSuccess || query_pass_b(geo, &p->info_b) != cudaSuccess ||
+        query_pass_c(geo, &p->info_c) != cudaSuccess)
         return bail(fail(p, EXX_ERR_INTERNAL, "no kernel instantiation for this geometry"));
 
     for (int ax = 0; ax < 3; ++ax) {
@@ -474,6 +514,22 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
         }
         if (cudaMemcpy(p->tw[ax], tw.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(p->roots[ax], roots.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(p, EXX_ERR_CUDA, "twiddle upload failed"));
+        }
+    }
+    {   // twb[b2*R1 + q] = W_TB^{b2 q}: twiddle between the two stages of the b-axis FFT (passes A and C)
+        int r1 = 0, r2 = 0;
+        bsplit_of(p->t[1], &r1, &r2);
+        std::vector<double2> tw, roots, twb(static_cast<size_t>(r1) * r2);
+        host_tables(p->t[1], tw, roots);
+        for (int b2 = 0; b2 < r2; ++b2)
+            for (int q = 0; q < r1; ++q) twb[static_cast<size_t>(b2) * r1 + q] = roots[(b2 * q) % p->t[1]];
+        if (cudaMalloc(&p->twb, twb.size() * sizeof(double2)) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(p, EXX_ERR_ALLOC, "cudaMalloc(twiddles) failed"));
+        }
+        if (cudaMemcpy(p->twb, twb.data(), twb.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess) {
             cudaGetLastError();
             return bail(fail(p, EXX_ERR_CUDA, "twiddle upload failed"));
         }
@@ -500,7 +556,7 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
         return bail(fail(p, EXX_ERR_ALLOC, "allocation of plan buffers failed"));
     }
     p->fixed_bytes = n * n * sizeof(double) + n * sizeof(double) + p->desc_cap * sizeof(XformDesc) +
-                     sizeof(double) * (static_cast<size_t>(p->t[0] / 2 + 1) * (p->t[1] / 2 + 1) * (p->t[2] / 2 + 1));
+                     sizeof(double) * (static_cast<size_t>(p->t[0] / 2 + 1) * (p->t[1] / 2 + 1) * p->t[2]);
     if (cudaMemset(p->e_mat, 0, n * n * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
         return bail(fail(p, EXX_ERR_CUDA, "cudaMemset failed"));
@@ -517,6 +573,7 @@ exx_status exx_plan_destroy(exx_plan* p) {
         if (p->roots[ax]) cudaFree(p->roots[ax]);
     }
     if (p->ks) cudaFree(p->ks);
+    if (p->twb) cudaFree(p->twb);
     free_workspace(p);
     if (p->e_mat) cudaFree(p->e_mat);
     if (p->occ_dev) cudaFree(p->occ_dev);

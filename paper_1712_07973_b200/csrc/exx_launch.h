@@ -11,13 +11,14 @@ namespace exx {
 struct Geometry {
     int ta, tb, tc;      // transform lengths (n periodic, 2n free)
     int free_bc;         // 0 periodic, 1 free
-    int chunk_log2;      // W1 layout parameter (CHUNK = 2 or 4)
+    int chunk;           // W1 layout parameter (CHUNK = 2 or 4), = chunk_for(ta, tb, free_bc)
 };
 
 struct KernelInfo {     // what a launcher reports about the instantiation it dispatches to
     int threads;
     int smem_bytes;
-    int tiles;           // pass A/C: CTAs per transform (na * R2 / G);  pass B: CTAs per transform (R1 * TC / CHUNK)
+    int tiles;           // pass A / C: CTAs per launch (na * R2 / G);  pass B: blocks per transform (R1 * TC / CHUNK)
+    int ctas_per_sm;     // occupancy the launcher sized its grid for (pass B: persistent grid = SMs * this)
 };
 
 // Transform lengths the FFT covers.
@@ -27,57 +28,78 @@ bool length_supported(int t);
 bool geometry_supported(const Geometry& g);
 
 // Each returns cudaSuccess or the launch/attribute error.  count = transforms in the batch.
-cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, int count, cudaStream_t s, KernelInfo* info);
+cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info);
 cudaError_t launch_pass_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info);
 cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info);
 // Query only (no launch): fills info for the geometry.
-cudaError_t query_pass_ac(const Geometry& g, KernelInfo* info);
+cudaError_t query_pass_a(const Geometry& g, KernelInfo* info);
 cudaError_t query_pass_b(const Geometry& g, KernelInfo* info);
-
-// Default CHUNK (log2) for a geometry: the largest of {4,2} whose pass-B tile fits shared memory comfortably.
-int default_chunk_log2(int ta, int tb);
+cudaError_t query_pass_c(const Geometry& g, KernelInfo* info);
 
 // Compile-time tuning shared by the instantiation files -------------------------------------------------------
-constexpr int kMaxSmemC = 220 * 1024;                      // pass C: two work buffers + operand stages
+constexpr int kSmemPerSM = 227 * 1024;                     // usable shared memory per SM (and per CTA, opt-in)
+constexpr int kMaxSmemAC = 220 * 1024;                     // passes A / C: work buffer(s) + operand stages
+constexpr int kMaxSmemB = 224 * 1024;
 constexpr int round_up32(int x) { return (x + 31) / 32 * 32; }
+constexpr int imin(int a, int b) { return a < b ? a : b; }
+constexpr int imax(int a, int b) { return a > b ? a : b; }
 
-// bytes of pass-C shared memory for a tile of G b2-values with `nstg` operand stages (mirrors CfgAC)
+// bytes of dynamic shared memory of pass A (one work buffer) / pass C (two work buffers, R1 lines per b2) for a tile of
+// g b2-values with `nstg` operand stages (mirrors CfgAC)
 template <int TC, int TB, bool FREE>
-constexpr int smem_c_bytes(int g, int nstg) {
+constexpr int smem_ac_bytes(int g, int nstg, bool pass_c) {
     constexpr int PC = Split<TC>::P, QC = Split<TC>::Q, R1 = BSplit<TB>::R1;
     constexpr int NB1 = FREE ? R1 / 2 : R1, NC = FREE ? TC / 2 : TC;
     constexpr int ROW = PC * (QC | 1);
     constexpr int LS = NC + (((QC - NC % 16) % 16) + 16) % 16;
-    return 2 * g * (R1 * ROW + (g > 1 ? 4 : 0)) * 16 + nstg * 2 * g * NB1 * LS * 8;
+    const int work = g * ((pass_c ? R1 : NB1) * ROW + (g > 1 ? 4 : 0)) * 16;
+    return (pass_c ? 2 : 1) * work + nstg * 2 * g * NB1 * LS * 8;
 }
 
-// largest G dividing R2 with at most 256 epilogue items per tile whose pass-C tile fits shared memory
+// largest G dividing R2 with at most 256 (line, n2) items per tile whose tile fits shared memory
 template <int TC, int TB, bool FREE>
-constexpr int pick_g() {
+constexpr int pick_g(bool pass_c, int max_bytes) {
     constexpr int R2 = BSplit<TB>::R2;
     constexpr int items = (FREE ? BSplit<TB>::R1 / 2 : BSplit<TB>::R1) * Split<TC>::Q;
     int g = 1;
     for (int c = 1; c <= R2; ++c)
-        if (R2 % c == 0 && c * items <= 256 && smem_c_bytes<TC, TB, FREE>(c, 1) <= kMaxSmemC) g = c;
+        if (R2 % c == 0 && c * items <= 256 && smem_ac_bytes<TC, TB, FREE>(c, 1, pass_c) <= max_bytes) g = c;
     return g;
+}
+
+// resident CTAs per SM to compile for: limited by shared memory, by a register floor per thread, and by `cap`
+constexpr int pick_minb(int smem, int nt, int reg_floor, int cap) {
+    return imax(1, imin(imin(kSmemPerSM / (smem + 1024), 65536 / (nt * reg_floor)), cap));
 }
 
 template <int TC, int TB, bool FREE>
 struct TuneAC {
-    static constexpr int G = pick_g<TC, TB, FREE>();
-    using Cfg = CfgAC<TC, TB, FREE, G>;
-    static constexpr int NT = round_up32(Cfg::ITEMS_LINE_Q) < 32 ? 32 : round_up32(Cfg::ITEMS_LINE_Q);
-    // pass C: more threads than epilogue items when the b-stage (ITEMS_POS items) is wider (free BC)
-    static constexpr int NT_C = NT >= 256 ? NT : (Cfg::ITEMS_POS >= 256 ? 256 : (round_up32(Cfg::ITEMS_POS) > NT ? round_up32(Cfg::ITEMS_POS) : NT));
-    static constexpr int NSTG_C = smem_c_bytes<TC, TB, FREE>(G, 2) <= kMaxSmemC ? 2 : 1;
-    static constexpr int SMEM_C = smem_c_bytes<TC, TB, FREE>(G, NSTG_C);
+    static constexpr int CHUNK = chunk_for(TC, TB, FREE);
+    // ---- pass C
+    static constexpr int G_C = pick_g<TC, TB, FREE>(true, kMaxSmemAC / 2);
+    using CfgC = CfgAC<TC, TB, FREE, G_C, CHUNK>;
+    static constexpr int NT_C = imax(32, round_up32(imax(CfgC::ITEMS_LINE_Q, imin(CfgC::ITEMS_POS, 256))));
+    static constexpr int NSTG_C = smem_ac_bytes<TC, TB, FREE>(G_C, 2, true) <= kMaxSmemAC ? 2 : 1;
+    static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true);
+    static constexpr int MINB_C = pick_minb(SMEM_C, NT_C, 128, 4);
+    // ---- pass A
+    static constexpr int G_A = pick_g<TC, TB, FREE>(false, kMaxSmemAC / 3);
+    using CfgA = CfgAC<TC, TB, FREE, G_A, CHUNK>;
+    static constexpr int NT_A = imax(32, round_up32(imax(CfgA::ITEMS_LINE_Q, imin(CfgA::ITEMS_POS, 256))));
+    static constexpr int NSTG_A = 2;
+    static constexpr int SMEM_A = smem_ac_bytes<TC, TB, FREE>(G_A, NSTG_A, false);
+    static constexpr int MINB_A = pick_minb(SMEM_A, NT_A, 96, 4);
+    static_assert(SMEM_C <= kMaxSmemAC && SMEM_A <= kMaxSmemAC, "tile does not fit shared memory");
 };
 
 template <int TA, int TB, bool FREE, int CHUNK>
 struct TuneB {
     using Cfg = CfgB<TA, TB, FREE, CHUNK>;
+    static constexpr bool LAND = (Cfg::WORK_ELEMS + Cfg::LAND_ELEMS) * 16 <= kMaxSmemB;
+    static constexpr int SMEM = (Cfg::WORK_ELEMS + (LAND ? Cfg::LAND_ELEMS : 0)) * 16;
     static constexpr int half = round_up32(Cfg::ITEMS_Q / 2);
     static constexpr int NT = half < 64 ? 64 : (half > 512 ? 512 : half);
+    static constexpr bool FITS = SMEM <= kMaxSmemB;
 };
 
 }  // namespace exx

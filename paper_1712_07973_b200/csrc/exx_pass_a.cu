@@ -4,43 +4,53 @@
 
 namespace exx {
 
-template <int TC, int TB, bool FREE>
-static cudaError_t run_a(const ArgsAC& args, int count, cudaStream_t s, KernelInfo* info, bool launch) {
-    using T = TuneAC<TC, TB, FREE>;
-    using C = typename T::Cfg;
-    constexpr int smem = C::SMEM_ELEMS * static_cast<int>(sizeof(double2));
-    auto kern = pass_a_kernel<C, T::NT>;
-    if (info) { info->threads = T::NT; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; }
-    if (!launch) return cudaSuccess;
-    static bool attr_done = false;
-    if (!attr_done) {
+template <class K>
+static cudaError_t prepare(K kern, int smem, int nt, bool* done, int* ctas_per_sm) {
+    if (!*done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, nt, smem);
+        if (e != cudaSuccess) return e;
+        *done = true;
     }
-    dim3 grid(args.na * C::TILES_PER_A, count);
-    kern<<<grid, T::NT, smem, s>>>(args);
+    return cudaSuccess;
+}
+
+template <int TC, int TB, bool FREE>
+static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+    using T = TuneAC<TC, TB, FREE>;
+    using C = typename T::CfgA;
+    constexpr int smem = T::SMEM_A;
+    static_assert(smem == C::SMEM_A * 16 + T::NSTG_A * C::OP_DOUBLES * 8, "pass A shared memory");
+    auto kern = pass_a_kernel<C, T::NT_A, T::NSTG_A, T::MINB_A>;
+    static bool done = false;
+    static int occ = 0;
+    if (info) { info->threads = T::NT_A; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
+    if (!launch) return cudaSuccess;
+    cudaError_t e = prepare(kern, smem, T::NT_A, &done, &occ);
+    if (e != cudaSuccess) return e;
+    if (info) info->ctas_per_sm = occ;
+    kern<<<args.na * C::TILES_PER_A, T::NT_A, smem, s>>>(args);
     return cudaGetLastError();
 }
 
-static cudaError_t dispatch_a(const Geometry& g, const ArgsAC& args, int count, cudaStream_t s, KernelInfo* info, bool launch) {
+static cudaError_t dispatch_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
 #define X(TC_, TB_)                                                                                  \
     if (g.tc == TC_ && g.tb == TB_)                                                                  \
-        return g.free_bc ? run_a<TC_, TB_, true>(args, count, s, info, launch)                        \
-                         : run_a<TC_, TB_, false>(args, count, s, info, launch);
+        return g.free_bc ? run_a<TC_, TB_, true>(args, s, info, launch) : run_a<TC_, TB_, false>(args, s, info, launch);
     EXX_FOR_EACH_PAIR(X)
 #undef X
     return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, int count, cudaStream_t s, KernelInfo* info) {
-    return dispatch_a(g, args, count, s, info, true);
+cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
+    return dispatch_a(g, args, s, info, true);
 }
 
-cudaError_t query_pass_ac(const Geometry& g, KernelInfo* info) {
+cudaError_t query_pass_a(const Geometry& g, KernelInfo* info) {
     ArgsAC args{};
     args.na = g.free_bc ? g.ta / 2 : g.ta;
-    return dispatch_a(g, args, 0, nullptr, info, false);
+    return dispatch_a(g, args, nullptr, info, false);
 }
 
 }  // namespace exx

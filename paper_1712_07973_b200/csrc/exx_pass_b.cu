@@ -4,27 +4,50 @@
 
 namespace exx {
 
-constexpr int kMaxSmemB = 200 * 1024;
+template <class K>
+static cudaError_t prepare(K kern, int smem, int nt, bool* done, int* ctas_per_sm) {
+    if (!*done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, nt, smem);
+        if (e != cudaSuccess) return e;
+        *done = true;
+    }
+    return cudaSuccess;
+}
+
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+            cudaGetLastError();
+            n = 148;
+        }
+    }
+    return n;
+}
 
 template <int TA, int TB, bool FREE, int CHUNK>
-static cudaError_t run_b(const ArgsB& args, int count, cudaStream_t s, KernelInfo* info, bool launch) {
+static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, KernelInfo* info, bool launch) {
     using T = TuneB<TA, TB, FREE, CHUNK>;
     using C = typename T::Cfg;
-    constexpr int smem = C::SMEM_ELEMS * static_cast<int>(sizeof(double2));
-    if constexpr (smem > kMaxSmemB) {
-        return cudaErrorInvalidValue;                      // this CHUNK does not fit; the plan picks the other one
+    if constexpr (!T::FITS) {
+        return cudaErrorInvalidValue;
     } else {
-        auto kern = pass_b_kernel<C, T::NT>;
-        if (info) { info->threads = T::NT; info->smem_bytes = smem; info->tiles = C::R1 * args.npch; }
+        auto kern = pass_b_kernel<C, T::NT, T::LAND>;
+        static bool done = false;
+        static int occ = 0;
+        if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; }
         if (!launch) return cudaSuccess;
-        static bool attr_done = false;
-        if (!attr_done) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-            if (e != cudaSuccess) return e;
-            attr_done = true;
-        }
-        dim3 grid(C::R1 * args.npch, count);
-        kern<<<grid, T::NT, smem, s>>>(args);
+        cudaError_t e = prepare(kern, T::SMEM, T::NT, &done, &occ);
+        if (e != cudaSuccess) return e;
+        if (info) info->ctas_per_sm = occ;
+        ArgsB args = args_in;
+        args.ntiles = count * C::R1 * args.npch;
+        const int slots = sm_count() * (occ > 0 ? occ : 1);
+        const int grid = args.ntiles < slots ? args.ntiles : slots;
+        kern<<<grid, T::NT, T::SMEM, s>>>(args);
         return cudaGetLastError();
     }
 }
@@ -32,11 +55,8 @@ static cudaError_t run_b(const ArgsB& args, int count, cudaStream_t s, KernelInf
 static cudaError_t dispatch_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info, bool launch) {
 #define X(TA_, TB_)                                                                                              \
     if (g.ta == TA_ && g.tb == TB_) {                                                                            \
-        if (g.chunk_log2 == 2)                                                                                   \
-            return g.free_bc ? run_b<TA_, TB_, true, 4>(args, count, s, info, launch)                             \
-                             : run_b<TA_, TB_, false, 4>(args, count, s, info, launch);                           \
-        return g.free_bc ? run_b<TA_, TB_, true, 2>(args, count, s, info, launch)                                 \
-                         : run_b<TA_, TB_, false, 2>(args, count, s, info, launch);                               \
+        if (g.free_bc) return run_b<TA_, TB_, true, chunk_for(TA_, TB_, true)>(args, count, s, info, launch);     \
+        return run_b<TA_, TB_, false, chunk_for(TA_, TB_, false)>(args, count, s, info, launch);                  \
     }
     EXX_FOR_EACH_PAIR(X)
 #undef X
@@ -49,15 +69,8 @@ cudaError_t launch_pass_b(const Geometry& g, const ArgsB& args, int count, cudaS
 
 cudaError_t query_pass_b(const Geometry& g, KernelInfo* info) {
     ArgsB args{};
-    args.npch = g.tc >> g.chunk_log2;
+    args.npch = g.tc / g.chunk;
     return dispatch_b(g, args, 0, nullptr, info, false);
-}
-
-int default_chunk_log2(int ta, int tb) {
-    Geometry g{ta, tb, 16, 0, 2};
-    KernelInfo info{};
-    if (query_pass_b(g, &info) == cudaSuccess && info.smem_bytes <= 100 * 1024) return 2;
-    return 1;
 }
 
 bool length_supported(int t) {

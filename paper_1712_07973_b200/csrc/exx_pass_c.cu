@@ -4,32 +4,53 @@
 
 namespace exx {
 
-template <int TC, int TB, bool FREE>
-static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
-    using T = TuneAC<TC, TB, FREE>;
-    using C = typename T::Cfg;
-    constexpr int NSTG = T::NSTG_C;                          // operand stages (psi_j, psi_l lines in flight)
-    constexpr int smem = T::SMEM_C;
-    static_assert(smem == (2 * C::SMEM_C * 16 + NSTG * C::OP_DOUBLES * 8) && smem <= kMaxSmemC, "pass C shared memory");
-    auto kern = pass_c_kernel<C, T::NT_C, NSTG>;
-    if (info) { info->threads = T::NT_C; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; }
-    static bool attr_done = false;
-    if (!attr_done) {
+template <class K>
+static cudaError_t prepare(K kern, int smem, int nt, bool* done, int* ctas_per_sm) {
+    if (!*done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, nt, smem);
+        if (e != cudaSuccess) return e;
+        *done = true;
     }
+    return cudaSuccess;
+}
+
+template <int TC, int TB, bool FREE>
+static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+    using T = TuneAC<TC, TB, FREE>;
+    using C = typename T::CfgC;
+    constexpr int smem = T::SMEM_C;
+    static_assert(smem == 2 * C::SMEM_C * 16 + T::NSTG_C * C::OP_DOUBLES * 8, "pass C shared memory");
+    auto kern = pass_c_kernel<C, T::NT_C, T::NSTG_C, T::MINB_C>;
+    static bool done = false;
+    static int occ = 0;
+    if (info) { info->threads = T::NT_C; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
+    if (!launch) return cudaSuccess;
+    cudaError_t e = prepare(kern, smem, T::NT_C, &done, &occ);
+    if (e != cudaSuccess) return e;
+    if (info) info->ctas_per_sm = occ;
     kern<<<args.na * C::TILES_PER_A, T::NT_C, smem, s>>>(args);
     return cudaGetLastError();
 }
 
-cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
-#define X(TC_, TB_)                                                                \
-    if (g.tc == TC_ && g.tb == TB_)                                                \
-        return g.free_bc ? run_c<TC_, TB_, true>(args, s, info) : run_c<TC_, TB_, false>(args, s, info);
+static cudaError_t dispatch_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+#define X(TC_, TB_)                                                                                  \
+    if (g.tc == TC_ && g.tb == TB_)                                                                  \
+        return g.free_bc ? run_c<TC_, TB_, true>(args, s, info, launch) : run_c<TC_, TB_, false>(args, s, info, launch);
     EXX_FOR_EACH_PAIR(X)
 #undef X
     return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
+    return dispatch_c(g, args, s, info, true);
+}
+
+cudaError_t query_pass_c(const Geometry& g, KernelInfo* info) {
+    ArgsAC args{};
+    args.na = g.free_bc ? g.ta / 2 : g.ta;
+    return dispatch_c(g, args, nullptr, info, false);
 }
 
 }  // namespace exx

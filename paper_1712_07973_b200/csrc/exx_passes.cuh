@@ -12,7 +12,6 @@
 //   pass C  (inverse + "Kernel 3"): inverse R1 stage along b, inverse FFT along c, then
 //           K psi_i += -(f_j V_ij psi_j + f_l V_il psi_l), K psi_j += -f_i V_ij psi_i, K psi_l += -f_i V_il psi_i,
 //           and block-reduced partial sums of rho_ij V_ij (PAPER.md:67-69 Eq. 3, :81-82 Eq. 5).
-//           One CTA owns a grid tile for ALL transforms of a same-i batch, so K psi_i accumulates in registers.
 //
 // 1-D FFT of length T = P*Q inside a tile (in place in shared memory, output in digit-scrambled order):
 //     n = Q n1 + n2,  k = k1 + P k2,   position p = k1*Q + k2 holds X[k]
@@ -21,9 +20,16 @@
 // scramble.  Free boundary conditions (Hockney padding to 2n) prune the zero half of every first stage and the
 // discarded half of every last stage.
 //
-// Every phase is written as a per-work-item function usable on host and device: the kernels run the items
-// strided over the CTA's threads with __syncthreads() between phases; tests/emu runs the very same item
-// functions sequentially on the CPU to validate the index algebra without a GPU.
+// Data movement (exx_async.cuh): all three kernels are software-pipelined loops.  Passes A and C: one CTA owns a
+// grid tile for ALL transforms of a same-i batch (psi_i and the K psi_i accumulator of its points stay in
+// registers); psi_j / psi_l lines arrive by TMA bulk copies into shared-memory stages one or two transforms
+// ahead; pass C gathers the W1 tile of the next transform with cp.async while it computes the current one and
+// sends the K psi_j / K psi_l increments out as TMA bulk reduce-adds.  Pass B: persistent CTAs; the next
+// [a][b2][pin] block lands by TMA bulk row copies while the current one is transformed.
+//
+// Every phase is split into an *_index function (thread -> shared/global offsets; evaluated ONCE per thread,
+// outside the loops) and a *_compute function (pure arithmetic on those offsets).  Both are __host__ __device__:
+// tests/emu runs the very same functions sequentially on the CPU to validate the index algebra without a GPU.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -52,17 +58,21 @@ template <> struct BSplit<128> { static constexpr int R1 = 16, R2 = 8;  };
 template <> struct BSplit<192> { static constexpr int R1 = 16, R2 = 12; };
 template <> struct BSplit<256> { static constexpr int R1 = 16, R2 = 16; };
 
+constexpr int r2_of(int tb) {
+    return tb == 16 ? 4 : tb == 32 ? 4 : tb == 64 ? 8 : tb == 96 ? 12 : tb == 128 ? 8 : tb == 192 ? 12 : 16;
+}
+// W1 stores CHUNK consecutive (scrambled) c-positions contiguously: 4 where the pass-B landing + work buffers of a
+// (TA x R2 x 4)-point block fit shared memory, else 2.  Non-cubic grids are limited to lengths <= 64, where the
+// answer is 4 for every combination, so passes A/C may evaluate it with TA := TC.
+constexpr int chunk_for(int ta, int tb, bool free_bc) {
+    return (free_bc ? 3 : 4) * (ta / 2) * (r2_of(tb) * 4 + 4) * 16 <= 200 * 1024 ? 4 : 2;
+}
+
 // One packed transform of a same-i batch: pairs (i,j) and (i,l); l < 0 = the imaginary slot is empty.
 struct XformDesc {
     int j, l;
     double fj, fl;
 };
-
-// Workspace W1 element index: [t][q][pch][a][b2][pin]  (pass B reads/writes contiguous [a][b2][pin] blocks).
-template <int R1, int R2>
-EXX_HD size_t w1_index(int t, int q, int pch, int a, int b2, int pin, int npch, int na, int chunk) {
-    return ((((static_cast<size_t>(t) * R1 + q) * npch + pch) * na + a) * R2 + b2) * chunk + pin;
-}
 
 EXX_HD double2 ld_ro(const double2* p) {
 #ifdef __CUDA_ARCH__
@@ -92,9 +102,9 @@ EXX_HD void cmul_conj(double& xr, double& xi, double2 w) {
 }
 
 // ---------------------------------------------------------------------------------------- pass A / C geometry
-template <int TC_, int TB_, bool FREE_, int G_>
+template <int TC_, int TB_, bool FREE_, int G_, int CHUNK_>
 struct CfgAC {
-    static constexpr int TC = TC_, TB = TB_, G = G_;
+    static constexpr int TC = TC_, TB = TB_, G = G_, CHUNK = CHUNK_;
     static constexpr bool FREE = FREE_;
     static constexpr int PC = Split<TC>::P, QC = Split<TC>::Q;
     static constexpr int R1 = BSplit<TB>::R1, R2 = BSplit<TB>::R2;
@@ -102,27 +112,35 @@ struct CfgAC {
     static constexpr int NB = FREE ? TB / 2 : TB;          // grid points along b
     static constexpr int NB1 = FREE ? R1 / 2 : R1;         // non-zero lines (b1) per (a,b2) tile
     static constexpr int PCN = FREE ? PC / 2 : PC;         // non-zero n1 per line
+    static constexpr int NPCH = TC / CHUNK;
     static constexpr int QCP = QC | 1;                     // padded row of the [k1][n2] layout (bank conflicts)
     static constexpr int ROW = PC * QCP;                   // shared-memory elements per line
-    static constexpr int LINES = G * NB1;
-    static constexpr int SMEM_ELEMS = LINES * ROW;
+    static constexpr int LINES = G * NB1;                  // real-space lines of the tile
     static constexpr int TILES_PER_A = R2 / G;             // CTAs per a-plane
     static constexpr int ITEMS_LINE_Q = LINES * QC;        // (line, n2) items: phases A0, C2
     static constexpr int ITEMS_LINE_P = LINES * PC;        // (line, k1) items: phases A1, C1
-    static constexpr int ITEMS_POS = G * TC;               // (g, position) items: phases A2, C0
+    static constexpr int ITEMS_POS = G * TC;               // (gi, position) columns: phases A2, C0
     static_assert(R2 % G == 0, "G must divide R2");
-    EXX_HD static int spos(int p) { return (p / QC) * QCP + (p % QC); }
-    // ---- pass C (v2): the W1 tile lands in place in the work buffer, which therefore has R1 lines per b2 of the tile
-    static constexpr int GPAD = G > 1 ? 4 : 0;             // shifts consecutive b2 groups by 64 B (bank conflicts)
-    static constexpr int GSTR_C = R1 * ROW + GPAD;         // elements between the line blocks of consecutive gi
-    static constexpr int SMEM_C = G * GSTR_C;              // elements of one pass-C work buffer
-    static constexpr int TILE_ELEMS = G * R1 * TC;         // complex values of one W1 tile
-    // operand lines (psi_j, psi_l; overwritten with the K psi_j, K psi_l increments) staged in shared memory:
-    // line stride LS doubles, LS = QC (mod 16) keeps the (line, n2)-mapped 8-byte accesses conflict-free
+    static_assert(TC % CHUNK == 0, "CHUNK must divide TC");
+    // work buffers: the lines of consecutive gi are GPAD elements (64 B) apart so that the (pin, gi)-ordered
+    // column accesses of A2 / C0 / the W1 gather hit disjoint banks
+    static constexpr int GPAD = G > 1 ? 4 : 0;
+    static constexpr int GSTR_A = NB1 * ROW + GPAD;        // pass A: NB1 lines per gi
+    static constexpr int SMEM_A = G * GSTR_A;
+    static constexpr int GSTR_C = R1 * ROW + GPAD;         // pass C: the W1 tile lands in place, R1 lines per gi
+    static constexpr int SMEM_C = G * GSTR_C;
+    // operand lines (psi_j, psi_l; pass C overwrites them with the K psi_j, K psi_l increments) staged in shared
+    // memory: line stride LS doubles, LS = QC (mod 16) keeps the (line, n2)-mapped 8-byte accesses conflict-free
     static constexpr int LS = NC + (((QC - NC % 16) % 16) + 16) % 16;
     static constexpr int OP_DOUBLES = 2 * LINES * LS;      // one stage: [slot j|l][line][LS]
+    static constexpr int LINE_BYTES = NC * 8;
     static_assert(LS % 2 == 0 && NC % 2 == 0, "16-byte alignment of operand lines");
-    EXX_HD static int line_c(int gi, int q) { return gi * GSTR_C + q * ROW; }
+    // W1 strides in elements ([t][q][pch][a][b2][pin], na = grid points along a)
+    EXX_HD static size_t w1_a() { return static_cast<size_t>(R2) * CHUNK; }
+    EXX_HD static size_t w1_pch(int na) { return static_cast<size_t>(na) * R2 * CHUNK; }
+    EXX_HD static size_t w1_q(int na) { return static_cast<size_t>(NPCH) * na * R2 * CHUNK; }
+    EXX_HD static size_t w1_t(int na) { return static_cast<size_t>(R1) * NPCH * na * R2 * CHUNK; }
+    EXX_HD static int spos(int p) { return (p / QC) * QCP + (p % QC); }
 };
 
 struct ArgsAC {
@@ -131,50 +149,89 @@ struct ArgsAC {
     double2* w1;
     const XformDesc* desc;      // first transform of this batch
     const double2* twc;         // [k1*QC + n2] = W_TC^{n2 k1}
-    const double2* rootsb;      // [m] = W_TB^m
+    const double2* twb;         // [b2*R1 + q]  = W_TB^{b2 q}
     double* epart;              // pass C: [count][ntiles][2] partial sums of rho*V
     long long m_points;         // na*nb*nc
     int na;
-    int chunk_log2;             // W1 layout: CHUNK = 1 << chunk_log2 contiguous c-positions per (a,b2)
     int i;                      // common orbital of the batch
     double fi;
     int count;                  // transforms in the batch
 };
 
-// ---- A0: co-density (Eq. 8) + zero padding + stage 1 of the c-axis FFT
+// Offset (doubles) of real-space line l = gi*NB1 + b1 of tile (a, b2base) inside one orbital.
 template <class C>
-EXX_HD void a0_item(int w, double2* S, const ArgsAC& g, const XformDesc& d, int a, int b2base) {
-    const int l = w / C::QC, n2 = w % C::QC;
+EXX_HD size_t line_offset(int l, int a, int b2base) {
     const int gi = l / C::NB1, b1 = l % C::NB1;
     const int b = C::R2 * b1 + b2base + gi;
-    const size_t base = (static_cast<size_t>(a) * C::NB + b) * C::NC + n2;
-    const double* pi = g.psi + static_cast<size_t>(g.i) * g.m_points + base;
-    const double* pj = g.psi + static_cast<size_t>(d.j) * g.m_points + base;
-    const double* pl = g.psi + static_cast<size_t>(d.l < 0 ? d.j : d.l) * g.m_points + base;
-    const double lmask = d.l < 0 ? 0.0 : 1.0;
+    return (static_cast<size_t>(a) * C::NB + b) * C::NC;
+}
+
+// ---- (line, n2) items of A0 / C2: work-buffer row offset, operand offset, global offset of the item's first point
+struct LineQIdx { int row; int op; int n2; size_t gofs; };
+template <class C, bool PASS_C>
+EXX_HD LineQIdx lineq_index(int w, int a, int b2base) {
+    const int l = w / C::QC, n2 = w % C::QC;
+    const int gi = l / C::NB1, b1 = l % C::NB1;
+    LineQIdx x;
+    x.row = gi * (PASS_C ? C::GSTR_C : C::GSTR_A) + b1 * C::ROW + n2;
+    x.op = l * C::LS + n2;
+    x.n2 = n2;
+    x.gofs = line_offset<C>(l, a, b2base) + n2;
+    return x;
+}
+
+// ---- (line, k1) items of A1 / C1: offset of the [k1] segment of the line, and k1 (twiddle row)
+struct LinePIdx { int seg; int k1; };
+template <class C, bool PASS_C>
+EXX_HD LinePIdx linep_index(int w) {
+    const int l = w / C::PC, k1 = w % C::PC;
+    const int gi = l / C::NB1, b1 = l % C::NB1;
+    LinePIdx x;
+    x.seg = gi * (PASS_C ? C::GSTR_C : C::GSTR_A) + b1 * C::ROW + k1 * C::QCP;
+    x.k1 = k1;
+    return x;
+}
+
+// ---- column items of A2 / C0 / the W1 gather, enumerated (pch, gi, pin) with pin fastest, then gi: consecutive
+//      items are consecutive in W1 for G*CHUNK elements (128 B for G*CHUNK = 8), so warp accesses coalesce.
+struct ColIdx { int col; int b2; size_t w1; };     // work-buffer column offset, b2, W1 offset at (t = 0, q = 0)
+template <class C, bool PASS_C>
+EXX_HD ColIdx col_index(int w, int a, int b2base, int na) {
+    const int pin = w % C::CHUNK;
+    const int gi = (w / C::CHUNK) % C::G;
+    const int pch = w / (C::CHUNK * C::G);
+    ColIdx x;
+    x.col = gi * (PASS_C ? C::GSTR_C : C::GSTR_A) + C::spos(pch * C::CHUNK + pin);
+    x.b2 = b2base + gi;
+    x.w1 = pch * C::w1_pch(na) + a * C::w1_a() + static_cast<size_t>(x.b2) * C::CHUNK + pin;
+    return x;
+}
+
+// ---------------------------------------------------------------------------------------- pass A phases
+// ---- A0: co-density (Eq. 8) + zero padding + stage 1 of the c-axis FFT.
+//      vi = psi_i at the item's PCN points; pj / pl = psi_j / psi_l at the item's first point, stride QC doubles
+//      between the points; row = work-buffer row of the item; tw = twc + n2.
+template <class C>
+EXX_HD void a0_compute(const double* vi, const double* pj, const double* pl, double lmask, double2* row, const double2* tw) {
     double xr[C::PC], xi[C::PC];
 #pragma unroll
     for (int n1 = 0; n1 < C::PCN; ++n1) {
-        const double vi = ld_ro(pi + C::QC * n1);
-        xr[n1] = vi * ld_ro(pj + C::QC * n1);
-        xi[n1] = vi * ld_ro(pl + C::QC * n1) * lmask;
+        xr[n1] = vi[n1] * pj[C::QC * n1];
+        xi[n1] = vi[n1] * pl[C::QC * n1] * lmask;
     }
 #pragma unroll
     for (int n1 = C::PCN; n1 < C::PC; ++n1) { xr[n1] = 0.0; xi[n1] = 0.0; }
     dft_fwd<C::PC, C::FREE>(xr, xi);
-    double2* row = S + l * C::ROW + n2;
 #pragma unroll
     for (int k1 = 0; k1 < C::PC; ++k1) {
-        if (k1 > 0) cmul(xr[k1], xi[k1], ld_ro(g.twc + k1 * C::QC + n2));
+        if (k1 > 0) cmul(xr[k1], xi[k1], ld_ro(tw + k1 * C::QC));
         row[k1 * C::QCP] = make_double2(xr[k1], xi[k1]);
     }
 }
 
 // ---- A1: stage 2 of the c-axis FFT (in place; the item reads and writes only its own row segment)
 template <class C>
-EXX_HD void a1_item(int w, double2* S) {
-    const int l = w / C::PC, k1 = w % C::PC;
-    double2* seg = S + l * C::ROW + k1 * C::QCP;
+EXX_HD void a1_compute(double2* seg) {
     double xr[C::QC], xi[C::QC];
 #pragma unroll
     for (int n2 = 0; n2 < C::QC; ++n2) { double2 v = seg[n2]; xr[n2] = v.x; xi[n2] = v.y; }
@@ -183,90 +240,63 @@ EXX_HD void a1_item(int w, double2* S) {
     for (int k2 = 0; k2 < C::QC; ++k2) seg[k2] = make_double2(xr[k2], xi[k2]);
 }
 
-// ---- A2: stage 1 (R1-point) of the b-axis FFT + twiddle W_TB^{b2 q}, store to W1
+// ---- A2: stage 1 (R1-point) of the b-axis FFT + twiddle W_TB^{b2 q}, store to W1.
+//      col = work-buffer column; tw = twb + b2*R1; dst = W1 element (t, q = 0) of the column; qstride = C::w1_q(na)
 template <class C>
-EXX_HD void a2_item(int w, const double2* S, const ArgsAC& g, int t, int a, int b2base) {
-    const int gi = w / C::TC, p = w % C::TC;
-    const int b2 = b2base + gi;
-    const double2* col = S + gi * C::NB1 * C::ROW + C::spos(p);
+EXX_HD void a2_compute(const double2* col, const double2* tw, double2* dst, size_t qstride) {
     double xr[C::R1], xi[C::R1];
 #pragma unroll
     for (int b1 = 0; b1 < C::NB1; ++b1) { double2 v = col[b1 * C::ROW]; xr[b1] = v.x; xi[b1] = v.y; }
 #pragma unroll
     for (int b1 = C::NB1; b1 < C::R1; ++b1) { xr[b1] = 0.0; xi[b1] = 0.0; }
     dft_fwd<C::R1, C::FREE>(xr, xi);
-    const int chunk = 1 << g.chunk_log2;
-    const int pch = p >> g.chunk_log2, pin = p & (chunk - 1);
-    const int npch = C::TC >> g.chunk_log2;
 #pragma unroll
     for (int q = 0; q < C::R1; ++q) {
-        if (q > 0) cmul(xr[q], xi[q], ld_ro(g.rootsb + (b2 * q) % C::TB));
-        g.w1[w1_index<C::R1, C::R2>(t, q, pch, a, b2, pin, npch, g.na, chunk)] = make_double2(xr[q], xi[q]);
+        if (q > 0) cmul(xr[q], xi[q], ld_ro(tw + q));
+        dst[q * qstride] = make_double2(xr[q], xi[q]);
     }
 }
 
-// ---- C landing: element e of the W1 tile of (t, a, b2base) -> (index in W1, element offset in the work buffer).
-//      e enumerates (q, pch, gi, pin) with pin fastest, then gi: consecutive e are consecutive in W1 for G*CHUNK
-//      elements (128 B runs for G*CHUNK = 8), so a warp's 16-byte cp.async requests coalesce into full lines.
-template <class C>
-EXX_HD void c_land_map(int e, const ArgsAC& g, int t, int a, int b2base, size_t* src, int* dst) {
-    const int chunk = 1 << g.chunk_log2;
-    const int npch = C::TC >> g.chunk_log2;
-    const int pin = e & (chunk - 1);
-    int r = e >> g.chunk_log2;
-    const int gi = r % C::G; r /= C::G;
-    const int pch = r % npch;
-    const int q = r / npch;
-    *src = w1_index<C::R1, C::R2>(t, q, pch, a, b2base + gi, pin, npch, g.na, chunk);
-    *dst = C::line_c(gi, q) + C::spos(pch * chunk + pin);
-}
-
+// ---------------------------------------------------------------------------------------- pass C phases
 // ---- C0: conj twiddle + inverse R1 stage of the b axis, in place in the work buffer (q lines -> b1 lines)
 template <class C>
-EXX_HD void c0_item(int w, double2* S, const ArgsAC& g, int b2base) {
-    const int gi = w / C::TC, p = w % C::TC;
-    const int b2 = b2base + gi;
-    double2* col = S + C::line_c(gi, 0) + C::spos(p);
+EXX_HD void c0_compute(double2* col, const double2* tw) {
     double xr[C::R1], xi[C::R1];
 #pragma unroll
     for (int q = 0; q < C::R1; ++q) {
         double2 v = col[q * C::ROW];
         xr[q] = v.x; xi[q] = v.y;
-        if (q > 0) cmul_conj(xr[q], xi[q], ld_ro(g.rootsb + (b2 * q) % C::TB));
+        if (q > 0) cmul_conj(xr[q], xi[q], ld_ro(tw + q));
     }
     dft_inv<C::R1, C::FREE>(xr, xi);
 #pragma unroll
     for (int b1 = 0; b1 < C::NB1; ++b1) col[b1 * C::ROW] = make_double2(xr[b1], xi[b1]);
 }
 
-// ---- C1: inverse stage over k2 (Q-point) of the c axis + conj twiddle
+// ---- C1: inverse stage over k2 (Q-point) of the c axis + conj twiddle.  tw = twc + k1*QC
 template <class C>
-EXX_HD void c1_item(int w, double2* S, const ArgsAC& g) {
-    const int l = w / C::PC, k1 = w % C::PC;
-    double2* seg = S + C::line_c(l / C::NB1, l % C::NB1) + k1 * C::QCP;
+EXX_HD void c1_compute(double2* seg, const double2* tw, int k1) {
     double xr[C::QC], xi[C::QC];
 #pragma unroll
     for (int k2 = 0; k2 < C::QC; ++k2) { double2 v = seg[k2]; xr[k2] = v.x; xi[k2] = v.y; }
     dft_inv<C::QC, false>(xr, xi);
 #pragma unroll
     for (int n2 = 0; n2 < C::QC; ++n2) {
-        if (k1 > 0) cmul_conj(xr[n2], xi[n2], ld_ro(g.twc + k1 * C::QC + n2));
+        if (k1 > 0) cmul_conj(xr[n2], xi[n2], ld_ro(tw + n2));
         seg[n2] = make_double2(xr[n2], xi[n2]);
     }
 }
 
 // ---- C2: inverse stage over k1 (P-point) of the c axis, then "Kernel 3" for the PCN points
-//      c = QC n1 + n2 of line l that this item owns:
+//      c = QC n1 + n2 of the line that this item owns:
 //      acc   += f_j V_ij psi_j + f_l V_il psi_l                 (K psi_i -= acc after the batch)
 //      oj    <- -f_i V_ij psi_i ,  ol <- -f_i V_il psi_i         increments of K psi_j, K psi_l, written over the
 //               staged psi_j / psi_l values and added to K psi by the memory system   PAPER.md:67-69 Eq. 3, :111
 //      e1    += rho_ij V_ij,  e2 += rho_il V_il                                        PAPER.md:81-82 Eq. 5
-//      vi = psi_i at the item's points; oj / ol = operand lines of this item at offset n2 (stride QC between n1).
+//      vi = psi_i at the item's points; oj / ol = operand lines at the item's first point (stride QC doubles).
 template <class C>
-EXX_HD void c2_item(int w, const double2* S, const XformDesc& d, double fi, const double* vi /*[PCN]*/, double* oj,
-                    double* ol, double* acc /*[PCN]*/, double& e1, double& e2) {
-    const int l = w / C::QC, n2 = w % C::QC;
-    const double2* row = S + C::line_c(l / C::NB1, l % C::NB1) + n2;
+EXX_HD void c2_compute(const double2* row, const XformDesc& d, double fi, const double* vi /*[PCN]*/, double* oj,
+                       double* ol, double* acc /*[PCN]*/, double& e1, double& e2) {
     double xr[C::PC], xi[C::PC];
 #pragma unroll
     for (int k1 = 0; k1 < C::PC; ++k1) { double2 v = row[k1 * C::QCP]; xr[k1] = v.x; xi[k1] = v.y; }
@@ -280,24 +310,15 @@ EXX_HD void c2_item(int w, const double2* S, const XformDesc& d, double fi, cons
         const double v1 = xr[n1], v2 = xi[n1];
         const double vj = oj[off];
         const double vl = has_l ? ol[off] : 0.0;
-        acc[n1] += d.fj * v1 * vj + fl * v2 * vl;
-        oj[off] = -(fi * v1 * vi[n1]);
-        if (has_l) ol[off] = -(fi * v2 * vi[n1]);
-        s1 += vi[n1] * vj * v1;
-        s2 += vi[n1] * vl * v2;
+        const double a1 = v1 * vi[n1], a2 = v2 * vi[n1];     // V_ij psi_i, V_il psi_i
+        acc[n1] += d.fj * (v1 * vj) + fl * (v2 * vl);
+        oj[off] = -(fi * a1);
+        if (has_l) ol[off] = -(fi * a2);
+        s1 += a1 * vj;
+        s2 += a2 * vl;
     }
     e1 += s1;
     e2 += s2;
-}
-
-template <class C>
-EXX_HD void c_flush_item(int w, const ArgsAC& g, int a, int b2base, const double* acc) {
-    const int l = w / C::QC, n2 = w % C::QC;
-    const int gi = l / C::NB1, b1 = l % C::NB1;
-    const int b = C::R2 * b1 + b2base + gi;
-    double* ki = g.kpsi + static_cast<size_t>(g.i) * g.m_points + (static_cast<size_t>(a) * C::NB + b) * C::NC + n2;
-#pragma unroll
-    for (int n1 = 0; n1 < C::PCN; ++n1) ki[C::QC * n1] -= acc[n1];
 }
 
 // ---------------------------------------------------------------------------------------- pass B geometry
@@ -312,7 +333,10 @@ struct CfgB {
     static constexpr int COLS = R2 * CHUNK;
     // row stride == CHUNK (mod 8) elements keeps the (a,pin)-mapped phases B0/B4 conflict-free
     static constexpr int RS = COLS + ((CHUNK - COLS % 8) + 8) % 8;
-    static constexpr int SMEM_ELEMS = TA * RS;
+    static constexpr int WORK_ELEMS = TA * RS;             // work buffer (all TA rows)
+    static constexpr int LAND_ELEMS = NA * RS;             // landing buffer (the NA rows that exist in W1)
+    static constexpr int ROW_BYTES = COLS * 16;            // one [b2][pin] row of W1
+    static constexpr int BLOCK_ELEMS = NA * COLS;          // one contiguous [a][b2][pin] block of W1
     static constexpr int ITEMS_IO = NA * CHUNK;            // (a, pin): B0, B4
     static constexpr int ITEMS_Q = COLS * QA;              // (n2, col): B1, B3
     static constexpr int ITEMS_P = COLS * PA;              // (k1, col): B2
@@ -321,91 +345,109 @@ struct CfgB {
 struct ArgsB {
     double2* w1;
     const double2* twa;         // [k1*QA + n2] = W_TA^{n2 k1}
-    const double* ks;           // symmetric Fourier kernel [TA/2+1][TB/2+1][TC/2+1], includes 1/T_tot (and dV)
-    int tc, pc, qc;             // c-axis transform length and its split (to unscramble kc)
-    int npch;
+    const double* ks;           // Fourier kernel [TA/2+1][TB/2+1][tc]: symmetric index along a and b, SCRAMBLED
+                                // position p along c (the order pass B meets it); includes 1/T_tot (and dV)
+    int tc;                     // c-axis transform length
+    int npch;                   // tc / CHUNK
+    int ntiles;                 // count * R1 * npch blocks in this launch
 };
 
+// (a, pin) items of B0 / B4: offset in the landing / work buffers (stride CHUNK between b2 resp. r) and in the W1 block
+struct IoIdx { int s; int g; };
 template <class C>
-EXX_HD void b0_item(int w, double2* S, const ArgsB& g, int t, int q, int pch) {
+EXX_HD IoIdx io_index(int w) {
     const int a = w / C::CHUNK, pin = w % C::CHUNK;
+    IoIdx x;
+    x.s = a * C::RS + pin;
+    x.g = a * C::COLS + pin;
+    return x;
+}
+// (n2, col) items of B1 / B3 and (k1, col) items of B2
+struct ColAIdx { int base; int k; int col; };
+template <class C>
+EXX_HD ColAIdx colq_index(int w) {                        // rows QA*n1 + n2, n1 = 0..PA-1
+    ColAIdx x;
+    x.col = w % C::COLS; x.k = w / C::COLS;
+    x.base = x.k * C::RS + x.col;
+    return x;
+}
+template <class C>
+EXX_HD ColAIdx colp_index(int w) {                        // rows k1*QA + n2, n2 = 0..QA-1
+    ColAIdx x;
+    x.col = w % C::COLS; x.k = w / C::COLS;
+    x.base = x.k * C::QA * C::RS + x.col;
+    return x;
+}
+
+// ---- B0: second (R2-point) stage of the b-axis FFT: src (landing buffer or W1 block) -> work buffer
+template <class C>
+EXX_HD void b0_compute(const double2* src, double2* dst) {
     double xr[C::R2], xi[C::R2];
-    const double2* src = g.w1 + w1_index<C::R1, C::R2>(t, q, pch, a, 0, pin, g.npch, C::NA, C::CHUNK);
 #pragma unroll
     for (int b2 = 0; b2 < C::R2; ++b2) { double2 v = src[b2 * C::CHUNK]; xr[b2] = v.x; xi[b2] = v.y; }
     Dft<C::R2>::run(xr, xi);
-    double2* dst = S + a * C::RS + pin;
 #pragma unroll
     for (int r = 0; r < C::R2; ++r) dst[r * C::CHUNK] = make_double2(xr[r], xi[r]);
 }
 
+// ---- B1: stage 1 of the a-axis FFT (P-point over n1, zero-padded half pruned) + twiddle.  tw = twa + n2
 template <class C>
-EXX_HD void b1_item(int w, double2* S, const ArgsB& g) {
-    const int col = w % C::COLS, n2 = w / C::COLS;
+EXX_HD void b1_compute(double2* colp, const double2* tw) {
     double xr[C::PA], xi[C::PA];
 #pragma unroll
-    for (int n1 = 0; n1 < C::PAN; ++n1) { double2 v = S[(C::QA * n1 + n2) * C::RS + col]; xr[n1] = v.x; xi[n1] = v.y; }
+    for (int n1 = 0; n1 < C::PAN; ++n1) { double2 v = colp[C::QA * n1 * C::RS]; xr[n1] = v.x; xi[n1] = v.y; }
 #pragma unroll
     for (int n1 = C::PAN; n1 < C::PA; ++n1) { xr[n1] = 0.0; xi[n1] = 0.0; }
     dft_fwd<C::PA, C::FREE>(xr, xi);
 #pragma unroll
     for (int k1 = 0; k1 < C::PA; ++k1) {
-        if (k1 > 0) cmul(xr[k1], xi[k1], ld_ro(g.twa + k1 * C::QA + n2));
-        S[(k1 * C::QA + n2) * C::RS + col] = make_double2(xr[k1], xi[k1]);
+        if (k1 > 0) cmul(xr[k1], xi[k1], ld_ro(tw + k1 * C::QA));
+        colp[k1 * C::QA * C::RS] = make_double2(xr[k1], xi[k1]);
     }
 }
 
-// B2: last forward stage along a, multiply by K^ ("convolving the density with the appropriate
-// Green's function"), first inverse stage along a.
+// ---- B2: last forward stage along a, multiply by K^ ("convolving the density with the appropriate
+//      Green's function"), first inverse stage along a.  kcol = ks + sb*tc + p of this column; kstride = (TB/2+1)*tc;
+//      tw = twa + k1*QA.
 template <class C>
-EXX_HD void b2_item(int w, double2* S, const ArgsB& g, int q, int pch) {
-    const int col = w % C::COLS, k1 = w / C::COLS;
+EXX_HD void b2_compute(double2* colp, const double* kcol, size_t kstride, const double2* tw, int k1) {
     double xr[C::QA], xi[C::QA];
 #pragma unroll
-    for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = S[(k1 * C::QA + n2) * C::RS + col]; xr[n2] = v.x; xi[n2] = v.y; }
+    for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = colp[n2 * C::RS]; xr[n2] = v.x; xi[n2] = v.y; }
     Dft<C::QA>::run(xr, xi);
-    const int r = col / C::CHUNK, pin = col % C::CHUNK;
-    const int kb = q + C::R1 * r;
-    const int p = pch * C::CHUNK + pin;
-    const int kc = (p / g.qc) + g.pc * (p % g.qc);
-    const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-    const int sc = kc <= g.tc - kc ? kc : g.tc - kc;
-    const int nbh = C::TB / 2 + 1, nch = g.tc / 2 + 1;
 #pragma unroll
     for (int k2 = 0; k2 < C::QA; ++k2) {
         const int ka = k1 + C::PA * k2;
         const int sa = ka <= C::TA - ka ? ka : C::TA - ka;
-        const double kv = ld_ro(g.ks + (static_cast<size_t>(sa) * nbh + sb) * nch + sc);
+        const double kv = ld_ro(kcol + sa * kstride);
         xr[k2] *= kv; xi[k2] *= kv;
     }
     dft_inv<C::QA, false>(xr, xi);
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) {
-        if (k1 > 0) cmul_conj(xr[n2], xi[n2], ld_ro(g.twa + k1 * C::QA + n2));
-        S[(k1 * C::QA + n2) * C::RS + col] = make_double2(xr[n2], xi[n2]);
+        if (k1 > 0) cmul_conj(xr[n2], xi[n2], ld_ro(tw + n2));
+        colp[n2 * C::RS] = make_double2(xr[n2], xi[n2]);
     }
 }
 
+// ---- B3: last inverse stage along a (outputs beyond the grid pruned)
 template <class C>
-EXX_HD void b3_item(int w, double2* S) {
-    const int col = w % C::COLS, n2 = w / C::COLS;
+EXX_HD void b3_compute(double2* colp) {
     double xr[C::PA], xi[C::PA];
 #pragma unroll
-    for (int k1 = 0; k1 < C::PA; ++k1) { double2 v = S[(k1 * C::QA + n2) * C::RS + col]; xr[k1] = v.x; xi[k1] = v.y; }
+    for (int k1 = 0; k1 < C::PA; ++k1) { double2 v = colp[k1 * C::QA * C::RS]; xr[k1] = v.x; xi[k1] = v.y; }
     dft_inv<C::PA, C::FREE>(xr, xi);
 #pragma unroll
-    for (int n1 = 0; n1 < C::PAN; ++n1) S[(C::QA * n1 + n2) * C::RS + col] = make_double2(xr[n1], xi[n1]);
+    for (int n1 = 0; n1 < C::PAN; ++n1) colp[C::QA * n1 * C::RS] = make_double2(xr[n1], xi[n1]);
 }
 
+// ---- B4: inverse R2 stage of the b axis: work buffer -> W1 block
 template <class C>
-EXX_HD void b4_item(int w, const double2* S, const ArgsB& g, int t, int q, int pch) {
-    const int a = w / C::CHUNK, pin = w % C::CHUNK;
+EXX_HD void b4_compute(const double2* src, double2* dst) {
     double xr[C::R2], xi[C::R2];
-    const double2* src = S + a * C::RS + pin;
 #pragma unroll
     for (int r = 0; r < C::R2; ++r) { double2 v = src[r * C::CHUNK]; xr[r] = v.x; xi[r] = v.y; }
     dft_inv<C::R2, false>(xr, xi);
-    double2* dst = g.w1 + w1_index<C::R1, C::R2>(t, q, pch, a, 0, pin, g.npch, C::NA, C::CHUNK);
 #pragma unroll
     for (int b2 = 0; b2 < C::R2; ++b2) dst[b2 * C::CHUNK] = make_double2(xr[b2], xi[b2]);
 }
@@ -413,53 +455,179 @@ EXX_HD void b4_item(int w, const double2* S, const ArgsB& g, int t, int q, int p
 // ---------------------------------------------------------------------------------------- kernels
 #ifdef __CUDACC__
 
-template <class C, int NT>
-__global__ void __launch_bounds__(NT) pass_a_kernel(const ArgsAC g) {
-    extern __shared__ double2 S[];
-    const int tile = blockIdx.x, t = blockIdx.y;
-    const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
-    const XformDesc d = g.desc[t];
-    for (int w = threadIdx.x; w < C::ITEMS_LINE_Q; w += NT) a0_item<C>(w, S, g, d, a, b2base);
-    __syncthreads();
-    for (int w = threadIdx.x; w < C::ITEMS_LINE_P; w += NT) a1_item<C>(w, S);
-    __syncthreads();
-    for (int w = threadIdx.x; w < C::ITEMS_POS; w += NT) a2_item<C>(w, S, g, t, a, b2base);
+__host__ __device__ constexpr int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// TMA bulk loads of the psi_j / psi_l lines of one transform into an operand stage (all 32 lanes of warp 0 call this)
+template <class C>
+__device__ __forceinline__ void issue_operand_loads(const ArgsAC& g, const XformDesc& d, double* stage, uint64_t* bar, int a,
+                                                    int b2base, int lane) {
+    const int nops = (d.l >= 0 ? 2 : 1) * C::LINES;
+    if (lane == 0) mbar_arrive_expect_tx(bar, nops * C::LINE_BYTES);
+    __syncwarp();
+    for (int o = lane; o < nops; o += 32) {
+        const int slot = o / C::LINES, l = o % C::LINES;
+        const double* src = g.psi + static_cast<size_t>(slot ? d.l : d.j) * g.m_points + line_offset<C>(l, a, b2base);
+        bulk_g2s(stage + (slot * C::LINES + l) * C::LS, src, C::LINE_BYTES, bar);
+    }
 }
 
-template <class C, int NT>
-__global__ void __launch_bounds__(NT) pass_b_kernel(const ArgsB g) {
-    extern __shared__ double2 S[];
-    const int q = blockIdx.x % C::R1, pch = blockIdx.x / C::R1, t = blockIdx.y;
-    for (int w = threadIdx.x; w < C::ITEMS_IO; w += NT) b0_item<C>(w, S, g, t, q, pch);
+// Pass A.  One CTA per (a, b2-group) tile, looping over the transforms of the same-i batch.  psi_i of the thread's
+// points lives in registers; psi_j / psi_l lines arrive NSTG transforms ahead by TMA bulk copies.
+template <class C, int NT, int NSTG, int MINB>
+__global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* const S = reinterpret_cast<double2*>(smem_raw);
+    double* const OP = reinterpret_cast<double*>(S + C::SMEM_A);
+    __shared__ uint64_t full[NSTG];
+    const int tile = blockIdx.x, tid = threadIdx.x;
+    const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
+    constexpr int NI0 = ceil_div(C::ITEMS_LINE_Q, NT), NI1 = ceil_div(C::ITEMS_LINE_P, NT), NI2 = ceil_div(C::ITEMS_POS, NT);
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
     __syncthreads();
-    for (int w = threadIdx.x; w < C::ITEMS_Q; w += NT) b1_item<C>(w, S, g);
+    if (tid < 32)
+        for (int t = 0; t < NSTG && t < g.count; ++t)
+            issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+
+    // per-thread items, resolved once
+    LineQIdx q0[NI0];
+    double vi[NI0][C::PCN];
+#pragma unroll
+    for (int m = 0; m < NI0; ++m) {
+        const int w = tid + m * NT;
+        q0[m] = lineq_index<C, false>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
+        const double* pi = g.psi + static_cast<size_t>(g.i) * g.m_points + q0[m].gofs;
+#pragma unroll
+        for (int n1 = 0; n1 < C::PCN; ++n1) vi[m][n1] = ld_ro(pi + C::QC * n1);
+    }
+    LinePIdx p1[NI1];
+#pragma unroll
+    for (int m = 0; m < NI1; ++m) p1[m] = linep_index<C, false>(tid + m * NT < C::ITEMS_LINE_P ? tid + m * NT : 0);
+    ColIdx c2[NI2];
+#pragma unroll
+    for (int m = 0; m < NI2; ++m) c2[m] = col_index<C, false>(tid + m * NT < C::ITEMS_POS ? tid + m * NT : 0, a, b2base, g.na);
+    const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
+
+    for (int t = 0; t < g.count; ++t) {
+        const int s = t % NSTG;
+        double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
+        const XformDesc d = g.desc[t];
+        const double lmask = d.l < 0 ? 0.0 : 1.0;
+        const int lofs = d.l < 0 ? 0 : C::LINES * C::LS;       // empty imaginary slot: read psi_j, multiply by 0
+        mbar_wait(&full[s], (t / NSTG) & 1);
+#pragma unroll
+        for (int m = 0; m < NI0; ++m)
+            if (tid + m * NT < C::ITEMS_LINE_Q)
+                a0_compute<C>(vi[m], stage + q0[m].op, stage + lofs + q0[m].op, lmask, S + q0[m].row, g.twc + q0[m].n2);
+        __syncthreads();
+        if (tid < 32 && t + NSTG < g.count)                    // the stage has been consumed: refill it
+            issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+#pragma unroll
+        for (int m = 0; m < NI1; ++m)
+            if (tid + m * NT < C::ITEMS_LINE_P) a1_compute<C>(S + p1[m].seg);
+        __syncthreads();
+        double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
+#pragma unroll
+        for (int m = 0; m < NI2; ++m)
+            if (tid + m * NT < C::ITEMS_POS) a2_compute<C>(S + c2[m].col, g.twb + c2[m].b2 * C::R1, w1t + c2[m].w1, qstride);
+        __syncthreads();
+    }
+}
+
+// Pass B.  Persistent CTAs over the (t, pch, q) blocks of the launch.  LAND: the next block lands in a separate
+// buffer by TMA bulk row copies while the current one is transformed; otherwise the block is loaded into the work
+// buffer itself (no overlap; only for geometries whose two buffers do not fit shared memory).
+template <class C, int NT, bool LAND>
+__global__ void __launch_bounds__(NT, 1) pass_b_kernel(const ArgsB g) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* const W = reinterpret_cast<double2*>(smem_raw);
+    double2* const L = LAND ? W + C::WORK_ELEMS : W;
+    __shared__ uint64_t full;
+    const int tid = threadIdx.x;
+    constexpr int NIO = ceil_div(C::ITEMS_IO, NT), NQ = ceil_div(C::ITEMS_Q, NT), NP = ceil_div(C::ITEMS_P, NT);
+
+    if (tid == 0) { mbar_init(&full, 1); mbar_fence_init(); }
     __syncthreads();
-    for (int w = threadIdx.x; w < C::ITEMS_P; w += NT) b2_item<C>(w, S, g, q, pch);
-    __syncthreads();
-    for (int w = threadIdx.x; w < C::ITEMS_Q; w += NT) b3_item<C>(w, S);
-    __syncthreads();
-    for (int w = threadIdx.x; w < C::ITEMS_IO; w += NT) b4_item<C>(w, S, g, t, q, pch);
+    auto block_ptr = [&](int id) -> double2* {             // id -> (t, pch, q), q fastest
+        const int q = id % C::R1, rest = id / C::R1;
+        const int pch = rest % g.npch, t = rest / g.npch;
+        return g.w1 + ((static_cast<size_t>(t) * C::R1 + q) * g.npch + pch) * C::BLOCK_ELEMS;
+    };
+    auto issue_block_load = [&](int id) {                  // all lanes of warp 0
+        const double2* src = block_ptr(id);
+        if (tid == 0) mbar_arrive_expect_tx(&full, C::NA * C::ROW_BYTES);
+        __syncwarp();
+        for (int a = tid; a < C::NA; a += 32) bulk_g2s(L + a * C::RS, src + a * C::COLS, C::ROW_BYTES, &full);
+    };
+    if (tid < 32 && static_cast<int>(blockIdx.x) < g.ntiles) issue_block_load(blockIdx.x);
+
+    IoIdx io[NIO];
+#pragma unroll
+    for (int m = 0; m < NIO; ++m) io[m] = io_index<C>(tid + m * NT < C::ITEMS_IO ? tid + m * NT : 0);
+    ColAIdx cq[NQ];
+#pragma unroll
+    for (int m = 0; m < NQ; ++m) cq[m] = colq_index<C>(tid + m * NT < C::ITEMS_Q ? tid + m * NT : 0);
+    ColAIdx cp[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) cp[m] = colp_index<C>(tid + m * NT < C::ITEMS_P ? tid + m * NT : 0);
+    const size_t kstride = static_cast<size_t>(C::TB / 2 + 1) * g.tc;
+
+    int it = 0;
+    for (int id = blockIdx.x; id < g.ntiles; id += gridDim.x, ++it) {
+        const int q = id % C::R1, pch = (id / C::R1) % g.npch;
+        double2* blk = block_ptr(id);
+        mbar_wait(&full, it & 1);
+#pragma unroll
+        for (int m = 0; m < NIO; ++m)
+            if (tid + m * NT < C::ITEMS_IO) b0_compute<C>(L + io[m].s, W + io[m].s);
+        __syncthreads();
+        if (LAND && tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
+#pragma unroll
+        for (int m = 0; m < NQ; ++m)
+            if (tid + m * NT < C::ITEMS_Q) b1_compute<C>(W + cq[m].base, g.twa + cq[m].k);
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < NP; ++m)
+            if (tid + m * NT < C::ITEMS_P) {
+                const int r = cp[m].col / C::CHUNK, pin = cp[m].col % C::CHUNK;
+                const int kb = q + C::R1 * r;
+                const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
+                b2_compute<C>(W + cp[m].base, g.ks + static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin, kstride,
+                              g.twa + cp[m].k * C::QA, cp[m].k);
+            }
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < NQ; ++m)
+            if (tid + m * NT < C::ITEMS_Q) b3_compute<C>(W + cq[m].base);
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < NIO; ++m)
+            if (tid + m * NT < C::ITEMS_IO) b4_compute<C>(W + io[m].s, blk + io[m].g);
+        __syncthreads();
+        if (!LAND && tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
+    }
 }
 
 // Pass C.  One CTA per (a, b2-group) tile; it loops over the transforms of the same-i batch, keeps the K psi_i
 // accumulator and psi_i of its points in registers, and is software-pipelined:
-//   * the W1 tile of transform t+1 is gathered into the second work buffer with 16-byte cp.async while t is computed;
+//   * every thread gathers the W1 columns it will transform (C0) for transform t+1 into the second work buffer with
+//     16-byte cp.async while t is computed (128-byte runs, see col_index);
 //   * psi_j / psi_l lines arrive NSTG transforms ahead by TMA bulk copies (mbarrier completion) into operand stages;
 //   * the K psi_j / K psi_l increments overwrite those lines and leave by TMA bulk reduce-add (fp64) -- each K psi
 //     address receives exactly one add per launch (the j of a batch are distinct), so the result is deterministic.
-// NT >= ITEMS_LINE_Q (one epilogue item per thread).
-template <class C, int NT, int NSTG>
-__global__ void __launch_bounds__(NT, 1) pass_c_kernel(const ArgsAC g) {
-    static_assert(NT >= C::ITEMS_LINE_Q, "pass C needs one thread per epilogue item");
+template <class C, int NT, int NSTG, int MINB>
+__global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* const S0 = reinterpret_cast<double2*>(smem_raw);
     double* const OP = reinterpret_cast<double*>(S0 + 2 * C::SMEM_C);
     __shared__ uint64_t full[NSTG];
     __shared__ double red[2][NT / 32];
-    const int tile = blockIdx.x;
+    const int tile = blockIdx.x, tid = threadIdx.x;
     const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
-    const int tid = threadIdx.x;
-    constexpr uint32_t LINE_BYTES = C::NC * sizeof(double);
+    constexpr int NI0 = ceil_div(C::ITEMS_POS, NT), NI1 = ceil_div(C::ITEMS_LINE_P, NT), NI2 = ceil_div(C::ITEMS_LINE_Q, NT);
 
     if (tid == 0) {
         for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
@@ -467,47 +635,38 @@ __global__ void __launch_bounds__(NT, 1) pass_c_kernel(const ArgsAC g) {
     }
     __syncthreads();
 
-    // operand traffic of transform t (warp 0): loads of psi_j / psi_l lines, later reduce-adds of the increments
-    auto line_gmem = [&](int orb, int l) -> size_t {
-        const int gi = l / C::NB1, b1 = l % C::NB1;
-        const int b = C::R2 * b1 + b2base + gi;
-        return static_cast<size_t>(orb) * g.m_points + (static_cast<size_t>(a) * C::NB + b) * C::NC;
-    };
-    auto issue_operand_loads = [&](int t) {          // called by all lanes of warp 0
-        const XformDesc d = g.desc[t];
-        const int s = t % NSTG;
-        double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
-        const int nops = (d.l >= 0 ? 2 : 1) * C::LINES;
-        if (tid == 0) mbar_arrive_expect_tx(&full[s], nops * LINE_BYTES);
-        __syncwarp();
-        for (int o = tid; o < nops; o += 32) {
-            const int slot = o / C::LINES, l = o % C::LINES;
-            bulk_g2s(stage + (slot * C::LINES + l) * C::LS, g.psi + line_gmem(slot ? d.l : d.j, l), LINE_BYTES, &full[s]);
-        }
-    };
-    auto issue_w1_gather = [&](int t) {              // all threads
+    ColIdx c0[NI0];
+#pragma unroll
+    for (int m = 0; m < NI0; ++m) c0[m] = col_index<C, true>(tid + m * NT < C::ITEMS_POS ? tid + m * NT : 0, a, b2base, g.na);
+    const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
+    auto issue_w1_gather = [&](int t) {
         double2* dstbuf = S0 + (t & 1) * C::SMEM_C;
-        for (int e = tid; e < C::TILE_ELEMS; e += NT) {
-            size_t src; int dst;
-            c_land_map<C>(e, g, t, a, b2base, &src, &dst);
-            cp_async16(dstbuf + dst, g.w1 + src);
-        }
+        const double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
+#pragma unroll
+        for (int m = 0; m < NI0; ++m)
+            if (tid + m * NT < C::ITEMS_POS) {
+#pragma unroll
+                for (int q = 0; q < C::R1; ++q) cp_async16(dstbuf + c0[m].col + q * C::ROW, w1t + c0[m].w1 + q * qstride);
+            }
     };
-
     issue_w1_gather(0);
     cp_async_commit();
     if (tid < 32)
-        for (int t = 0; t < NSTG && t < g.count; ++t) issue_operand_loads(t);
+        for (int t = 0; t < NSTG && t < g.count; ++t)
+            issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
 
-    // this thread's epilogue item: PCN points of one line
-    const int my_l = tid / C::QC, my_n2 = tid % C::QC;
-    double vi[C::PCN], acc[C::PCN];
+    LinePIdx p1[NI1];
 #pragma unroll
-    for (int n1 = 0; n1 < C::PCN; ++n1) { vi[n1] = 0.0; acc[n1] = 0.0; }
-    if (tid < C::ITEMS_LINE_Q) {
-        const double* pi = g.psi + line_gmem(g.i, my_l) + my_n2;
+    for (int m = 0; m < NI1; ++m) p1[m] = linep_index<C, true>(tid + m * NT < C::ITEMS_LINE_P ? tid + m * NT : 0);
+    LineQIdx q2[NI2];
+    double vi[NI2][C::PCN], acc[NI2][C::PCN];
 #pragma unroll
-        for (int n1 = 0; n1 < C::PCN; ++n1) vi[n1] = ld_ro(pi + C::QC * n1);
+    for (int m = 0; m < NI2; ++m) {
+        const int w = tid + m * NT;
+        q2[m] = lineq_index<C, true>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
+        const double* pi = g.psi + static_cast<size_t>(g.i) * g.m_points + q2[m].gofs;
+#pragma unroll
+        for (int n1 = 0; n1 < C::PCN; ++n1) { vi[m][n1] = ld_ro(pi + C::QC * n1); acc[m][n1] = 0.0; }
     }
 
     for (int t = 0; t < g.count; ++t) {
@@ -517,18 +676,21 @@ __global__ void __launch_bounds__(NT, 1) pass_c_kernel(const ArgsAC g) {
         const XformDesc d = g.desc[t];
         if (t + 1 < g.count) issue_w1_gather(t + 1);
         cp_async_commit();
-        cp_async_wait<1>();                                // this thread's part of tile t has landed
+        cp_async_wait<1>();                                // this thread's columns of transform t have landed
+#pragma unroll
+        for (int m = 0; m < NI0; ++m)
+            if (tid + m * NT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, g.twb + c0[m].b2 * C::R1);
         __syncthreads();
-        for (int w = tid; w < C::ITEMS_POS; w += NT) c0_item<C>(w, S, g, b2base);
-        __syncthreads();
-        for (int w = tid; w < C::ITEMS_LINE_P; w += NT) c1_item<C>(w, S, g);
+#pragma unroll
+        for (int m = 0; m < NI1; ++m)
+            if (tid + m * NT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, g.twc + p1[m].k1 * C::QC, p1[m].k1);
         __syncthreads();
         mbar_wait(&full[s], (t / NSTG) & 1);               // psi_j / psi_l lines of transform t have landed
         double e1 = 0.0, e2 = 0.0;
-        if (tid < C::ITEMS_LINE_Q) {
-            double* oj = stage + my_l * C::LS + my_n2;
-            c2_item<C>(tid, S, d, g.fi, vi, oj, oj + C::LINES * C::LS, acc, e1, e2);
-        }
+#pragma unroll
+        for (int m = 0; m < NI2; ++m)
+            if (tid + m * NT < C::ITEMS_LINE_Q)
+                c2_compute<C>(S + q2[m].row, d, g.fi, vi[m], stage + q2[m].op, stage + C::LINES * C::LS + q2[m].op, acc[m], e1, e2);
         fence_proxy_async();                               // increments visible to the TMA reads below
         // block reduction of the energy partials in a fixed order (deterministic)
 #pragma unroll
@@ -551,17 +713,25 @@ __global__ void __launch_bounds__(NT, 1) pass_c_kernel(const ArgsAC g) {
             for (int o = tid; o < 2 * C::LINES; o += 32) {
                 const int slot = o / C::LINES, l = o % C::LINES;
                 if (slot ? upd_l : upd_j)
-                    bulk_red_add_f64(g.kpsi + line_gmem(slot ? d.l : d.j, l), stage + (slot * C::LINES + l) * C::LS, LINE_BYTES);
+                    bulk_red_add_f64(g.kpsi + static_cast<size_t>(slot ? d.l : d.j) * g.m_points + line_offset<C>(l, a, b2base),
+                                     stage + (slot * C::LINES + l) * C::LS, C::LINE_BYTES);
             }
             bulk_commit();
             if (t + NSTG < g.count) {
                 bulk_wait_read_all();                      // the stage may be overwritten
                 __syncwarp();
-                issue_operand_loads(t + NSTG);
+                issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
             }
         }
     }
-    if (tid < C::ITEMS_LINE_Q) c_flush_item<C>(tid, g, a, b2base, acc);
+    // K psi_i -= sum over the batch (this CTA is the only writer of its tile of K psi_i in this launch)
+#pragma unroll
+    for (int m = 0; m < NI2; ++m)
+        if (tid + m * NT < C::ITEMS_LINE_Q) {
+            double* ki = g.kpsi + static_cast<size_t>(g.i) * g.m_points + q2[m].gofs;
+#pragma unroll
+            for (int n1 = 0; n1 < C::PCN; ++n1) ki[C::QC * n1] -= acc[m][n1];
+        }
     if (tid < 32) bulk_wait_read_all();                    // shared memory must outlive the TMA reads
 }
 

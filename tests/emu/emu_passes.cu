@@ -12,75 +12,111 @@ using namespace exx;
 
 template <int TA, int TB, int TC, bool FREE, int G, int CHUNK>
 static int emu_batch(const double* psi, double* kpsi, int i, double fi, int count, const XformDesc* desc,
-                     const double2* twa, const double2* twc, const double2* rootsb, const double* ks,
+                     const double2* twa, const double2* twc, const double2* rootsb, const double* ks_sym,
                      double* e_out /*[count][2]*/) {
-    using AC = CfgAC<TC, TB, FREE, G>;
+    using AC = CfgAC<TC, TB, FREE, G, CHUNK>;
     static_assert(CHUNK == 2 || CHUNK == 4, "chunk");
     using B = CfgB<TA, TB, FREE, CHUNK>;
     const int na = B::NA;
     const long long m_points = static_cast<long long>(na) * AC::NB * AC::NC;
     std::vector<double2> w1(static_cast<size_t>(count) * na * TB * TC);
     const int ntiles = na * AC::TILES_PER_A;
-    std::vector<double> epart(static_cast<size_t>(count) * ntiles * 2, 0.0);
+    // tables the plan builds: twb[b2*R1+q] = W_TB^{b2 q};  K^ with the c index in scrambled order
+    std::vector<double2> twb(static_cast<size_t>(AC::R1) * AC::R2);
+    for (int b2 = 0; b2 < AC::R2; ++b2)
+        for (int q = 0; q < AC::R1; ++q) twb[b2 * AC::R1 + q] = rootsb[(b2 * q) % TB];
+    const int nah = TA / 2 + 1, nbh = TB / 2 + 1, nch = TC / 2 + 1;
+    std::vector<double> ks(static_cast<size_t>(nah) * nbh * TC);
+    for (int r = 0; r < nah * nbh; ++r)
+        for (int p = 0; p < TC; ++p) {
+            const int kc = (p / AC::QC) + AC::PC * (p % AC::QC);
+            ks[static_cast<size_t>(r) * TC + p] = ks_sym[static_cast<size_t>(r) * nch + (kc <= TC - kc ? kc : TC - kc)];
+        }
     ArgsAC g{};
-    g.psi = psi; g.kpsi = kpsi; g.w1 = w1.data(); g.desc = desc; g.twc = twc; g.rootsb = rootsb;
-    g.epart = epart.data(); g.m_points = m_points; g.na = na; g.chunk_log2 = CHUNK == 4 ? 2 : 1; g.i = i; g.fi = fi; g.count = count;
-    std::vector<double2> S(AC::SMEM_ELEMS > B::SMEM_ELEMS ? AC::SMEM_ELEMS : B::SMEM_ELEMS);
-    // pass A
-    for (int t = 0; t < count; ++t)
-        for (int tile = 0; tile < ntiles; ++tile) {
-            const int a = tile / AC::TILES_PER_A, b2base = (tile % AC::TILES_PER_A) * G;
-            for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) a0_item<AC>(w, S.data(), g, desc[t], a, b2base);
-            for (int w = 0; w < AC::ITEMS_LINE_P; ++w) a1_item<AC>(w, S.data());
-            for (int w = 0; w < AC::ITEMS_POS; ++w) a2_item<AC>(w, S.data(), g, t, a, b2base);
-        }
-    // pass B
-    ArgsB gb{};
-    gb.w1 = w1.data(); gb.twa = twa; gb.ks = ks; gb.tc = TC; gb.pc = Split<TC>::P; gb.qc = Split<TC>::Q;
-    gb.npch = TC / CHUNK;
-    for (int t = 0; t < count; ++t)
-        for (int blk = 0; blk < B::R1 * gb.npch; ++blk) {
-            const int q = blk % B::R1, pch = blk / B::R1;
-            for (int w = 0; w < B::ITEMS_IO; ++w) b0_item<B>(w, S.data(), gb, t, q, pch);
-            for (int w = 0; w < B::ITEMS_Q; ++w) b1_item<B>(w, S.data(), gb);
-            for (int w = 0; w < B::ITEMS_P; ++w) b2_item<B>(w, S.data(), gb, q, pch);
-            for (int w = 0; w < B::ITEMS_Q; ++w) b3_item<B>(w, S.data());
-            for (int w = 0; w < B::ITEMS_IO; ++w) b4_item<B>(w, S.data(), gb, t, q, pch);
-        }
-    // pass C (v2): W1 tile landed in place in the work buffer (c_land_map = the kernel's cp.async gather), psi_j / psi_l
-    // lines staged in an operand buffer that c2 overwrites with the K psi_j / K psi_l increments (the kernel's TMA
-    // bulk loads and bulk reduce-adds are plain copies / adds here).
-    std::vector<double2> SC(AC::SMEM_C);
+    g.psi = psi; g.kpsi = kpsi; g.w1 = w1.data(); g.desc = desc; g.twc = twc; g.twb = twb.data();
+    g.m_points = m_points; g.na = na; g.i = i; g.fi = fi; g.count = count;
+    const size_t qstride = AC::w1_q(na), tstride = AC::w1_t(na);
+    std::vector<double2> S(AC::SMEM_A), SC(AC::SMEM_C), W(B::WORK_ELEMS), L(B::LAND_ELEMS);
     std::vector<double> op(AC::OP_DOUBLES);
-    std::vector<double> acc(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN), vi(acc.size());
-    auto line_gmem = [&](int orb, int l, int a, int b2base) {
-        const int gi = l / AC::NB1, b1 = l % AC::NB1;
-        const int b = AC::R2 * b1 + b2base + gi;
-        return static_cast<size_t>(orb) * m_points + (static_cast<size_t>(a) * AC::NB + b) * AC::NC;
+    std::vector<double> vi(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN), acc(vi.size());
+    auto stage_operands = [&](const XformDesc& d, int a, int b2base) {      // the kernels' TMA bulk line loads
+        for (int slot = 0; slot < (d.l >= 0 ? 2 : 1); ++slot)
+            for (int l = 0; l < AC::LINES; ++l)
+                std::memcpy(&op[(slot * AC::LINES + l) * AC::LS],
+                            psi + static_cast<size_t>(slot ? d.l : d.j) * m_points + line_offset<AC>(l, a, b2base), AC::NC * sizeof(double));
     };
+    // pass A
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int a = tile / AC::TILES_PER_A, b2base = (tile % AC::TILES_PER_A) * G;
+        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
+            const LineQIdx x = lineq_index<AC, false>(w, a, b2base);
+            for (int n1 = 0; n1 < AC::PCN; ++n1) vi[static_cast<size_t>(w) * AC::PCN + n1] = psi[static_cast<size_t>(i) * m_points + x.gofs + AC::QC * n1];
+        }
+        for (int t = 0; t < count; ++t) {
+            const XformDesc d = desc[t];
+            stage_operands(d, a, b2base);
+            const double lmask = d.l < 0 ? 0.0 : 1.0;
+            const int lofs = d.l < 0 ? 0 : AC::LINES * AC::LS;
+            for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
+                const LineQIdx x = lineq_index<AC, false>(w, a, b2base);
+                a0_compute<AC>(&vi[static_cast<size_t>(w) * AC::PCN], &op[x.op], &op[lofs + x.op], lmask, S.data() + x.row, twc + x.n2);
+            }
+            for (int w = 0; w < AC::ITEMS_LINE_P; ++w) a1_compute<AC>(S.data() + linep_index<AC, false>(w).seg);
+            for (int w = 0; w < AC::ITEMS_POS; ++w) {
+                const ColIdx x = col_index<AC, false>(w, a, b2base, na);
+                a2_compute<AC>(S.data() + x.col, twb.data() + x.b2 * AC::R1, w1.data() + t * tstride + x.w1, qstride);
+            }
+        }
+    }
+    // pass B
+    const int npch = TC / CHUNK;
+    const size_t kstride = static_cast<size_t>(nbh) * TC;
+    for (int id = 0; id < count * B::R1 * npch; ++id) {
+        const int q = id % B::R1, pch = (id / B::R1) % npch, t = id / (B::R1 * npch);
+        double2* blk = w1.data() + ((static_cast<size_t>(t) * B::R1 + q) * npch + pch) * B::BLOCK_ELEMS;
+        for (int a = 0; a < B::NA; ++a) std::memcpy(&L[a * B::RS], blk + a * B::COLS, B::ROW_BYTES);   // TMA bulk row loads
+        for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b0_compute<B>(L.data() + x.s, W.data() + x.s); }
+        for (int w = 0; w < B::ITEMS_Q; ++w) { const ColAIdx x = colq_index<B>(w); b1_compute<B>(W.data() + x.base, twa + x.k); }
+        for (int w = 0; w < B::ITEMS_P; ++w) {
+            const ColAIdx x = colp_index<B>(w);
+            const int r = x.col / CHUNK, pin = x.col % CHUNK;
+            const int kb = q + B::R1 * r;
+            const int sb = kb <= TB - kb ? kb : TB - kb;
+            b2_compute<B>(W.data() + x.base, ks.data() + static_cast<size_t>(sb) * TC + pch * CHUNK + pin, kstride, twa + x.k * B::QA, x.k);
+        }
+        for (int w = 0; w < B::ITEMS_Q; ++w) b3_compute<B>(W.data() + colq_index<B>(w).base);
+        for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b4_compute<B>(W.data() + x.s, blk + x.g); }
+    }
+    // pass C: the W1 columns land in place in the work buffer (the kernel's cp.async gather), psi_j / psi_l lines are
+    // staged in an operand buffer that C2 overwrites with the K psi_j / K psi_l increments (the kernel's TMA bulk
+    // loads and bulk reduce-adds are plain copies / adds here).
     for (int tile = 0; tile < ntiles; ++tile) {
         const int a = tile / AC::TILES_PER_A, b2base = (tile % AC::TILES_PER_A) * G;
         std::fill(acc.begin(), acc.end(), 0.0);
-        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w)
-            for (int n1 = 0; n1 < AC::PCN; ++n1)
-                vi[static_cast<size_t>(w) * AC::PCN + n1] = psi[line_gmem(i, w / AC::QC, a, b2base) + w % AC::QC + AC::QC * n1];
+        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
+            const LineQIdx x = lineq_index<AC, true>(w, a, b2base);
+            for (int n1 = 0; n1 < AC::PCN; ++n1) vi[static_cast<size_t>(w) * AC::PCN + n1] = psi[static_cast<size_t>(i) * m_points + x.gofs + AC::QC * n1];
+        }
         for (int t = 0; t < count; ++t) {
-            for (int e = 0; e < AC::TILE_ELEMS; ++e) {
-                size_t src; int dst;
-                c_land_map<AC>(e, g, t, a, b2base, &src, &dst);
-                SC[dst] = w1[src];
+            for (int w = 0; w < AC::ITEMS_POS; ++w) {
+                const ColIdx x = col_index<AC, true>(w, a, b2base, na);
+                for (int q = 0; q < AC::R1; ++q) SC[x.col + q * AC::ROW] = w1[t * tstride + x.w1 + q * qstride];
             }
-            for (int w = 0; w < AC::ITEMS_POS; ++w) c0_item<AC>(w, SC.data(), g, b2base);
-            for (int w = 0; w < AC::ITEMS_LINE_P; ++w) c1_item<AC>(w, SC.data(), g);
+            for (int w = 0; w < AC::ITEMS_POS; ++w) {
+                const ColIdx x = col_index<AC, true>(w, a, b2base, na);
+                c0_compute<AC>(SC.data() + x.col, twb.data() + x.b2 * AC::R1);
+            }
+            for (int w = 0; w < AC::ITEMS_LINE_P; ++w) {
+                const LinePIdx x = linep_index<AC, true>(w);
+                c1_compute<AC>(SC.data() + x.seg, twc + x.k1 * AC::QC, x.k1);
+            }
             const XformDesc d = desc[t];
-            for (int slot = 0; slot < (d.l >= 0 ? 2 : 1); ++slot)
-                for (int l = 0; l < AC::LINES; ++l)
-                    std::memcpy(&op[(slot * AC::LINES + l) * AC::LS], psi + line_gmem(slot ? d.l : d.j, l, a, b2base), AC::NC * sizeof(double));
+            stage_operands(d, a, b2base);
             double e1 = 0.0, e2 = 0.0;
             for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
-                double* oj = &op[(w / AC::QC) * AC::LS + w % AC::QC];
-                c2_item<AC>(w, SC.data(), d, fi, &vi[static_cast<size_t>(w) * AC::PCN], oj, oj + AC::LINES * AC::LS,
-                            &acc[static_cast<size_t>(w) * AC::PCN], e1, e2);
+                const LineQIdx x = lineq_index<AC, true>(w, a, b2base);
+                c2_compute<AC>(SC.data() + x.row, d, fi, &vi[static_cast<size_t>(w) * AC::PCN], &op[x.op], &op[AC::LINES * AC::LS + x.op],
+                               &acc[static_cast<size_t>(w) * AC::PCN], e1, e2);
             }
             e_out[2 * t] += e1;
             e_out[2 * t + 1] += e2;
@@ -88,11 +124,14 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
                 const int orb = slot ? d.l : d.j;
                 if (orb < 0 || orb == i) continue;
                 for (int l = 0; l < AC::LINES; ++l)
-                    for (int c = 0; c < AC::NC; ++c) kpsi[line_gmem(orb, l, a, b2base) + c] += op[(slot * AC::LINES + l) * AC::LS + c];
+                    for (int c = 0; c < AC::NC; ++c)
+                        kpsi[static_cast<size_t>(orb) * m_points + line_offset<AC>(l, a, b2base) + c] += op[(slot * AC::LINES + l) * AC::LS + c];
             }
         }
-        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w)
-            c_flush_item<AC>(w, g, a, b2base, acc.data() + static_cast<size_t>(w) * AC::PCN);
+        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
+            const LineQIdx x = lineq_index<AC, true>(w, a, b2base);
+            for (int n1 = 0; n1 < AC::PCN; ++n1) kpsi[static_cast<size_t>(i) * m_points + x.gofs + AC::QC * n1] -= acc[static_cast<size_t>(w) * AC::PCN + n1];
+        }
     }
     return 0;
 }
