@@ -79,18 +79,20 @@ __global__ void cos_transform_kernel(const double* in, double* out, long long ou
     }
 }
 
-// ks_perm[sa][sb][p] = ks_sym[sa][sb][sc(p)]: the c index in the digit-scrambled order of the in-tile FFT
-// (position p = k1*QC + k2 holds frequency kc = k1 + PC*k2), so that pass B reads K^ contiguously along pin.
-__global__ void permute_kernel_c_axis(const double* ks_sym, double* ks_perm, long long rows, int tc, int pc, int qc) {
+// ks_perm[sb][p][sa] = ks_sym[sa][sb][sc(p)]: the c index in the digit-scrambled order of the in-tile FFT
+// (position p = k1*QC + k2 holds frequency kc = k1 + PC*k2) and the symmetric a index fastest, so that the lanes of a
+// pass-B warp (consecutive k1 of one column) read K^ contiguously.
+__global__ void permute_kernel_axes(const double* ks_sym, double* ks_perm, int nah, int nbh, int tc, int pc, int qc) {
     const int nch = tc / 2 + 1;
-    const long long total = rows * tc;
+    const long long total = static_cast<long long>(nbh) * tc * nah;
     for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
          x += static_cast<long long>(gridDim.x) * blockDim.x) {
-        const int p = static_cast<int>(x % tc);
-        const long long row = x / tc;
+        const int sa = static_cast<int>(x % nah);
+        const int p = static_cast<int>((x / nah) % tc);
+        const int sb = static_cast<int>(x / (static_cast<long long>(nah) * tc));
         const int kc = (p / qc) + pc * (p % qc);
         const int sc = kc <= tc - kc ? kc : tc - kc;
-        ks_perm[x] = ks_sym[row * nch + sc];
+        ks_perm[x] = ks_sym[(static_cast<long long>(sa) * nbh + sb) * nch + sc];
     }
 }
 
@@ -155,7 +157,7 @@ struct exx_plan {
     double2* tw[3];
     double2* roots[3];
     double2* twb;           // [b2*R1 + q] = W_TB^{b2 q}
-    double* ks;             // [TA/2+1][TB/2+1][TC], c index in scrambled order
+    double* ks;             // [TB/2+1][TC][TA/2+1], c index in scrambled order (see permute_kernel_axes)
     double2* w1;
     size_t w1_elems_per_xform;
     double* epart;
@@ -299,7 +301,7 @@ exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
     auto permute = [&]() -> cudaError_t {
         int pc = 0, qc = 0;
         split_of(p->t[2], &pc, &qc);
-        permute_kernel_c_axis<<<2048, 256, 0, p->stream>>>(ks_sym, p->ks, static_cast<long long>(na) * nb, p->t[2], pc, qc);
+        permute_kernel_axes<<<2048, 256, 0, p->stream>>>(ks_sym, p->ks, na, nb, p->t[2], pc, qc);
         ++p->launches;
         cudaError_t e = cudaGetLastError();
         return e != cudaSuccess ? e : cudaStreamSynchronize(p->stream);

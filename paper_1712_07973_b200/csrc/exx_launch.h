@@ -39,7 +39,6 @@ cudaError_t query_pass_c(const Geometry& g, KernelInfo* info);
 // Compile-time tuning shared by the instantiation files -------------------------------------------------------
 constexpr int kSmemPerSM = 227 * 1024;                     // usable shared memory per SM (and per CTA, opt-in)
 constexpr int kMaxSmemAC = 220 * 1024;                     // passes A / C: work buffer(s) + operand stages
-constexpr int kMaxSmemB = 224 * 1024;
 constexpr int round_up32(int x) { return (x + 31) / 32 * 32; }
 constexpr int imin(int a, int b) { return a < b ? a : b; }
 constexpr int imax(int a, int b) { return a > b ? a : b; }
@@ -95,10 +94,10 @@ struct TuneAC {
 template <int TA, int TB, bool FREE, int CHUNK>
 struct TuneB {
     using Cfg = CfgB<TA, TB, FREE, CHUNK>;
-    static constexpr bool LAND = (Cfg::WORK_ELEMS + Cfg::LAND_ELEMS) * 16 <= kMaxSmemB;
-    static constexpr int SMEM = (Cfg::WORK_ELEMS + (LAND ? Cfg::LAND_ELEMS : 0)) * 16;
-    static constexpr int half = round_up32(Cfg::ITEMS_Q / 2);
-    static constexpr int NT = half < 64 ? 64 : (half > 512 ? 512 : half);
+    static constexpr int SMEM = Cfg::SMEM_BYTES;
+    // one warp per column group, at most 16 warps; small blocks share an SM (persistent grid = SMs * MINB)
+    static constexpr int NT = 32 * imin(Cfg::NGRP, 16);
+    static constexpr int MINB = imax(1, imin(imin(kSmemPerSM / (SMEM + 1024), 512 / NT), 8));
     static constexpr bool FITS = SMEM <= kMaxSmemB;
 };
 

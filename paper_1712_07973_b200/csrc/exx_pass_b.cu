@@ -35,7 +35,7 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
     if constexpr (!T::FITS) {
         return cudaErrorInvalidValue;
     } else {
-        auto kern = pass_b_kernel<C, T::NT, T::LAND>;
+        auto kern = pass_b_kernel<C, T::NT, T::MINB>;
         static bool done = false;
         static int occ = 0;
         if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; }
@@ -44,6 +44,7 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
         if (e != cudaSuccess) return e;
         if (info) info->ctas_per_sm = occ;
         ArgsB args = args_in;
+        args.count = count;
         args.ntiles = count * C::R1 * args.npch;
         const int slots = sm_count() * (occ > 0 ? occ : 1);
         const int grid = args.ntiles < slots ? args.ntiles : slots;

@@ -61,12 +61,9 @@ template <> struct BSplit<256> { static constexpr int R1 = 16, R2 = 16; };
 constexpr int r2_of(int tb) {
     return tb == 16 ? 4 : tb == 32 ? 4 : tb == 64 ? 8 : tb == 96 ? 12 : tb == 128 ? 8 : tb == 192 ? 12 : 16;
 }
-// W1 stores CHUNK consecutive (scrambled) c-positions contiguously: 4 where the pass-B landing + work buffers of a
-// (TA x R2 x 4)-point block fit shared memory, else 2.  Non-cubic grids are limited to lengths <= 64, where the
-// answer is 4 for every combination, so passes A/C may evaluate it with TA := TC.
-constexpr int chunk_for(int ta, int tb, bool free_bc) {
-    return (free_bc ? 3 : 4) * (ta / 2) * (r2_of(tb) * 4 + 4) * 16 <= 200 * 1024 ? 4 : 2;
-}
+constexpr int split_p(int t) { return t == 16 ? 4 : t == 32 ? 4 : t == 64 ? 8 : t == 96 ? 8 : t == 128 ? 8 : t == 192 ? 12 : 16; }
+constexpr int split_q(int t) { return t / split_p(t); }
+constexpr int chunk_for(int ta, int tb, bool free_bc);     // defined after the pass-B geometry helpers
 
 // One packed transform of a same-i batch: pairs (i,j) and (i,l); l < 0 = the imaginary slot is empty.
 struct XformDesc {
@@ -322,6 +319,97 @@ EXX_HD void c2_compute(const double2* row, const XformDesc& d, double fi, const 
 }
 
 // ---------------------------------------------------------------------------------------- pass B geometry
+// Shared-memory bank model for 16-byte accesses: a warp request is served quarter-warp by quarter-warp (8 lanes,
+// 128 bytes); lanes of a quarter that hit the same 16-byte bank group (offset mod 8) at different addresses
+// serialise.  wavefronts32() counts the wavefronts of one warp-wide access (4 = conflict-free).
+constexpr int wavefronts32(const int (&off)[32], int n_active) {
+    int total = 0;
+    for (int qw = 0; qw < 4; ++qw) {
+        int worst = 0;
+        for (int bank = 0; bank < 8; ++bank) {
+            int cnt = 0;
+            for (int l = 0; l < 8; ++l) {
+                const int lane = qw * 8 + l;
+                if (lane >= n_active || ((off[lane] % 8) + 8) % 8 != bank) continue;
+                bool dup = false;
+                for (int l2 = 0; l2 < l; ++l2)
+                    if (off[qw * 8 + l2] == off[lane]) dup = true;
+                if (!dup) ++cnt;
+            }
+            if (cnt > worst) worst = cnt;
+        }
+        total += worst;
+    }
+    return total;
+}
+
+// Work-buffer layout of pass B: element (row a, column col) at (a / QA) * QRS + (a % QA) * RS + col, QRS = QA*RS + PADK.
+// The three warp access patterns that must be conflict-free:
+//   io  (B0/B4): lane -> (a = lane / CHUNK, pin = lane % CHUNK)
+//   q   (B1/B3): lane -> (n2 = lane / NCW, cw = lane % NCW), rows QA*n1 + n2   -> offset n2*RS + cw  (+ n1*QRS)
+//   p   (B2)   : lane -> (k1 = lane / NCW, cw = lane % NCW), rows k1*QA + n2   -> offset k1*QRS + cw (+ n2*RS)
+constexpr int padb_cost(int rs, int padk, int qa, int pa, int ncw, int chunk) {
+    const int qrs = qa * rs + padk;
+    int o_io[32] = {}, o_q[32] = {}, o_p[32] = {};
+    for (int l = 0; l < 32; ++l) {
+        const int a = l / chunk;
+        o_io[l] = (a / qa) * qrs + (a % qa) * rs + l % chunk;
+        o_q[l] = (l / ncw) * rs + l % ncw;
+        o_p[l] = (l / ncw) * qrs + l % ncw;
+    }
+    const int nq = qa * ncw < 32 ? qa * ncw : 32, np = pa * ncw < 32 ? pa * ncw : 32;
+    return wavefronts32(o_io, 32) + 2 * wavefronts32(o_q, nq) + 2 * wavefronts32(o_p, np);
+}
+struct PadB { int rs, padk; };
+constexpr PadB pick_padb(int cols, int qa, int pa, int ncw, int chunk) {
+    PadB best{cols, 0};
+    int best_cost = 1 << 30;
+    for (int rs = cols; rs < cols + 8; ++rs)
+        for (int padk = 0; padk < 8; ++padk) {
+            const int c = padb_cost(rs, padk, qa, pa, ncw, chunk) * 1024 + (rs - cols) * 16 + padk;
+            if (c < best_cost) { best_cost = c; best = PadB{rs, padk}; }
+        }
+    return best;
+}
+// landing buffer: rows a*RSL, lanes (a, pin)
+constexpr int pick_rsl(int cols, int chunk) {
+    int best = cols, best_cost = 1 << 30;
+    for (int rs = cols; rs < cols + 8; ++rs) {
+        int o[32] = {};
+        for (int l = 0; l < 32; ++l) o[l] = (l / chunk) * rs + l % chunk;
+        const int c = wavefronts32(o, 32) * 1024 + (rs - cols);
+        if (c < best_cost) { best_cost = c; best = rs; }
+    }
+    return best;
+}
+// columns owned by one warp in the a-axis phases: the divisor of COLS that best fills the 32 lanes in B2 (PA*NCW
+// items, the heaviest phase) while leaving at least 8 column groups (warps) where possible; ties -> fewer columns
+constexpr int pick_ncw(int pa, int cols) {
+    int best = 1, best_score = -1;
+    for (int n = 1; n <= cols; ++n) {
+        if (cols % n != 0) continue;
+        const int items = pa * n, rounds = (items + 31) / 32, ngrp = cols / n;
+        const int score = items * 1000 / (32 * rounds) * (ngrp < 8 ? ngrp : 8);
+        if (score > best_score) { best_score = score; best = n; }
+    }
+    return best;
+}
+
+// bytes of dynamic shared memory of pass B for a [NA][R2][chunk] block (mirrors CfgB::SMEM_BYTES)
+constexpr int smem_b_bytes(int ta, int tb, bool free_bc, int chunk) {
+    const int pa = split_p(ta), qa = split_q(ta), cols = r2_of(tb) * chunk;
+    const int ncw = pick_ncw(pa, cols);
+    const PadB pad = pick_padb(cols, qa, pa, ncw, chunk);
+    return (pa * (qa * pad.rs + pad.padk) + (free_bc ? ta / 2 : ta) * pick_rsl(cols, chunk) + 2 * ta) * 16;
+}
+constexpr int kMaxSmemB = 224 * 1024;
+// W1 stores CHUNK consecutive (scrambled) c-positions contiguously: the largest of 4, 2, 1 for which the pass-B work +
+// landing buffers of a (TA x R2 x CHUNK)-point block fit shared memory.  Non-cubic grids are limited to lengths <= 64,
+// where the answer is 4 for every combination, so passes A/C may evaluate it with TA := TC.
+constexpr int chunk_for(int ta, int tb, bool free_bc) {
+    return smem_b_bytes(ta, tb, free_bc, 4) <= kMaxSmemB ? 4 : smem_b_bytes(ta, tb, free_bc, 2) <= kMaxSmemB ? 2 : 1;
+}
+
 template <int TA_, int TB_, bool FREE_, int CHUNK_>
 struct CfgB {
     static constexpr int TA = TA_, TB = TB_, CHUNK = CHUNK_;
@@ -331,55 +419,65 @@ struct CfgB {
     static constexpr int NA = FREE ? TA / 2 : TA;
     static constexpr int PAN = FREE ? PA / 2 : PA;
     static constexpr int COLS = R2 * CHUNK;
-    // row stride == CHUNK (mod 8) elements keeps the (a,pin)-mapped phases B0/B4 conflict-free
-    static constexpr int RS = COLS + ((CHUNK - COLS % 8) + 8) % 8;
-    static constexpr int WORK_ELEMS = TA * RS;             // work buffer (all TA rows)
-    static constexpr int LAND_ELEMS = NA * RS;             // landing buffer (the NA rows that exist in W1)
+    static constexpr int NCW = pick_ncw(PA, COLS);         // columns per warp (column group)
+    static constexpr int NGRP = COLS / NCW;                // column groups
+    static constexpr PadB PAD = pick_padb(COLS, QA, PA, NCW, CHUNK);
+    static constexpr int RS = PAD.rs;                      // row stride inside a block of QA rows
+    static constexpr int QRS = QA * RS + PAD.padk;         // stride between blocks of QA rows
+    static constexpr int RSL = pick_rsl(COLS, CHUNK);      // landing-buffer row stride
+    static constexpr int WORK_ELEMS = PA * QRS;            // work buffer (all TA rows)
+    static constexpr int LAND_ELEMS = NA * RSL;            // landing buffer (the NA rows that exist in W1)
     static constexpr int ROW_BYTES = COLS * 16;            // one [b2][pin] row of W1
     static constexpr int BLOCK_ELEMS = NA * COLS;          // one contiguous [a][b2][pin] block of W1
     static constexpr int ITEMS_IO = NA * CHUNK;            // (a, pin): B0, B4
-    static constexpr int ITEMS_Q = COLS * QA;              // (n2, col): B1, B3
-    static constexpr int ITEMS_P = COLS * PA;              // (k1, col): B2
+    static constexpr int ITEMS_Q = QA * NCW;               // (n2, cw) per column group: B1, B3
+    static constexpr int ITEMS_P = PA * NCW;               // (k1, cw) per column group: B2
+    static constexpr int NSA = TA / 2 + 1;                 // symmetric a-range of K^
+    static constexpr int SMEM_BYTES = (WORK_ELEMS + LAND_ELEMS + 2 * TA) * 16;
+    EXX_HD static int row_off(int a) { return (a / QA) * QRS + (a % QA) * RS; }
 };
 
 struct ArgsB {
     double2* w1;
     const double2* twa;         // [k1*QA + n2] = W_TA^{n2 k1}
-    const double* ks;           // Fourier kernel [TA/2+1][TB/2+1][tc]: symmetric index along a and b, SCRAMBLED
-                                // position p along c (the order pass B meets it); includes 1/T_tot (and dV)
+    const double* ks;           // Fourier kernel [TB/2+1][tc][TA/2+1]: symmetric index along b, SCRAMBLED position p
+                                // along c (the order pass B meets it), symmetric index along a fastest; includes
+                                // 1/T_tot (and dV)
     int tc;                     // c-axis transform length
     int npch;                   // tc / CHUNK
+    int count;                  // transforms in the batch
     int ntiles;                 // count * R1 * npch blocks in this launch
 };
 
-// (a, pin) items of B0 / B4: offset in the landing / work buffers (stride CHUNK between b2 resp. r) and in the W1 block
-struct IoIdx { int s; int g; };
+// (a, pin) items of B0 / B4: offsets in the landing buffer, the work buffer and the W1 block
+struct IoIdx { int l; int s; int g; };
 template <class C>
 EXX_HD IoIdx io_index(int w) {
     const int a = w / C::CHUNK, pin = w % C::CHUNK;
     IoIdx x;
-    x.s = a * C::RS + pin;
+    x.l = a * C::RSL + pin;
+    x.s = C::row_off(a) + pin;
     x.g = a * C::COLS + pin;
     return x;
 }
-// (n2, col) items of B1 / B3 and (k1, col) items of B2
+// items of the a-axis phases inside column group cg: B1/B3 item w -> (n2, cw), B2 item w -> (k1, cw)
 struct ColAIdx { int base; int k; int col; };
 template <class C>
-EXX_HD ColAIdx colq_index(int w) {                        // rows QA*n1 + n2, n1 = 0..PA-1
+EXX_HD ColAIdx colq_index(int cg, int w) {                // rows QA*n1 + n2, n1 = 0..PA-1 (stride QRS)
     ColAIdx x;
-    x.col = w % C::COLS; x.k = w / C::COLS;
+    x.k = w / C::NCW; x.col = cg * C::NCW + w % C::NCW;
     x.base = x.k * C::RS + x.col;
     return x;
 }
 template <class C>
-EXX_HD ColAIdx colp_index(int w) {                        // rows k1*QA + n2, n2 = 0..QA-1
+EXX_HD ColAIdx colp_index(int cg, int w) {                // rows k1*QA + n2, n2 = 0..QA-1 (stride RS)
     ColAIdx x;
-    x.col = w % C::COLS; x.k = w / C::COLS;
-    x.base = x.k * C::QA * C::RS + x.col;
+    x.k = w / C::NCW; x.col = cg * C::NCW + w % C::NCW;
+    x.base = x.k * C::QRS + x.col;
     return x;
 }
 
-// ---- B0: second (R2-point) stage of the b-axis FFT: src (landing buffer or W1 block) -> work buffer
+// ---- B0: second (R2-point) stage of the b-axis FFT: landing buffer -> work buffer (row a, all r, one pin)
 template <class C>
 EXX_HD void b0_compute(const double2* src, double2* dst) {
     double xr[C::R2], xi[C::R2];
@@ -390,27 +488,27 @@ EXX_HD void b0_compute(const double2* src, double2* dst) {
     for (int r = 0; r < C::R2; ++r) dst[r * C::CHUNK] = make_double2(xr[r], xi[r]);
 }
 
-// ---- B1: stage 1 of the a-axis FFT (P-point over n1, zero-padded half pruned) + twiddle.  tw = twa + n2
+// ---- B1: stage 1 of the a-axis FFT (P-point over n1, zero-padded half pruned) + twiddle W_TA^{n2 k1} = tw[k1*tws]
 template <class C>
-EXX_HD void b1_compute(double2* colp, const double2* tw) {
+EXX_HD void b1_compute(double2* colp, const double2* tw, int tws) {
     double xr[C::PA], xi[C::PA];
 #pragma unroll
-    for (int n1 = 0; n1 < C::PAN; ++n1) { double2 v = colp[C::QA * n1 * C::RS]; xr[n1] = v.x; xi[n1] = v.y; }
+    for (int n1 = 0; n1 < C::PAN; ++n1) { double2 v = colp[n1 * C::QRS]; xr[n1] = v.x; xi[n1] = v.y; }
 #pragma unroll
     for (int n1 = C::PAN; n1 < C::PA; ++n1) { xr[n1] = 0.0; xi[n1] = 0.0; }
     dft_fwd<C::PA, C::FREE>(xr, xi);
 #pragma unroll
     for (int k1 = 0; k1 < C::PA; ++k1) {
-        if (k1 > 0) cmul(xr[k1], xi[k1], ld_ro(tw + k1 * C::QA));
-        colp[k1 * C::QA * C::RS] = make_double2(xr[k1], xi[k1]);
+        if (k1 > 0) cmul(xr[k1], xi[k1], tw[k1 * tws]);
+        colp[k1 * C::QRS] = make_double2(xr[k1], xi[k1]);
     }
 }
 
 // ---- B2: last forward stage along a, multiply by K^ ("convolving the density with the appropriate
-//      Green's function"), first inverse stage along a.  kcol = ks + sb*tc + p of this column; kstride = (TB/2+1)*tc;
-//      tw = twa + k1*QA.
+//      Green's function"), first inverse stage along a.  kcol = K^ line [sa] of this column (symmetric a index);
+//      conj twiddle W_TA^{-n2 k1} = conj(tw[n2*tws]).
 template <class C>
-EXX_HD void b2_compute(double2* colp, const double* kcol, size_t kstride, const double2* tw, int k1) {
+EXX_HD void b2_compute(double2* colp, const double* kcol, const double2* tw, int tws, int k1) {
     double xr[C::QA], xi[C::QA];
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = colp[n2 * C::RS]; xr[n2] = v.x; xi[n2] = v.y; }
@@ -419,13 +517,13 @@ EXX_HD void b2_compute(double2* colp, const double* kcol, size_t kstride, const 
     for (int k2 = 0; k2 < C::QA; ++k2) {
         const int ka = k1 + C::PA * k2;
         const int sa = ka <= C::TA - ka ? ka : C::TA - ka;
-        const double kv = ld_ro(kcol + sa * kstride);
+        const double kv = ld_ro(kcol + sa);
         xr[k2] *= kv; xi[k2] *= kv;
     }
     dft_inv<C::QA, false>(xr, xi);
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) {
-        if (k1 > 0) cmul_conj(xr[n2], xi[n2], ld_ro(tw + n2));
+        if (k1 > 0) cmul_conj(xr[n2], xi[n2], tw[n2 * tws]);
         colp[n2 * C::RS] = make_double2(xr[n2], xi[n2]);
     }
 }
@@ -435,10 +533,10 @@ template <class C>
 EXX_HD void b3_compute(double2* colp) {
     double xr[C::PA], xi[C::PA];
 #pragma unroll
-    for (int k1 = 0; k1 < C::PA; ++k1) { double2 v = colp[k1 * C::QA * C::RS]; xr[k1] = v.x; xi[k1] = v.y; }
+    for (int k1 = 0; k1 < C::PA; ++k1) { double2 v = colp[k1 * C::QRS]; xr[k1] = v.x; xi[k1] = v.y; }
     dft_inv<C::PA, C::FREE>(xr, xi);
 #pragma unroll
-    for (int n1 = 0; n1 < C::PAN; ++n1) colp[C::QA * n1 * C::RS] = make_double2(xr[n1], xi[n1]);
+    for (int n1 = 0; n1 < C::PAN; ++n1) colp[n1 * C::QRS] = make_double2(xr[n1], xi[n1]);
 }
 
 // ---- B4: inverse R2 stage of the b axis: work buffer -> W1 block
@@ -537,77 +635,87 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     }
 }
 
-// Pass B.  Persistent CTAs over the (t, pch, q) blocks of the launch.  LAND: the next block lands in a separate
-// buffer by TMA bulk row copies while the current one is transformed; otherwise the block is loaded into the work
-// buffer itself (no overlap; only for geometries whose two buffers do not fit shared memory).
-template <class C, int NT, bool LAND>
-__global__ void __launch_bounds__(NT, 1) pass_b_kernel(const ArgsB g) {
+// Pass B.  Persistent CTAs over the (pch, q, t) blocks of the launch, t fastest (CTAs that run at the same time
+// share a K^ slice in L2).  The next block lands in a separate buffer by TMA bulk row copies while the current one is
+// transformed.  B0 / B4 map a thread to the rows (a, pin) it alone reads and writes, and the a-axis phases B1..B3 map
+// a WARP to the NCW columns it alone owns (only __syncwarp between them), so a block costs two CTA barriers:
+//     wait(landing) -> B0 -> barrier -> [issue next load] B1 ~ B2 ~ B3 -> barrier -> B4 -> next block.
+// The a-axis twiddles live in shared memory in both index orders ([k1*QA+n2] for B1, [n2*PA+k1] for B2).
+template <class C, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* const W = reinterpret_cast<double2*>(smem_raw);
-    double2* const L = LAND ? W + C::WORK_ELEMS : W;
+    double2* const L = W + C::WORK_ELEMS;
+    double2* const TW1 = L + C::LAND_ELEMS;
+    double2* const TW2 = TW1 + C::TA;
     __shared__ uint64_t full;
-    const int tid = threadIdx.x;
-    constexpr int NIO = ceil_div(C::ITEMS_IO, NT), NQ = ceil_div(C::ITEMS_Q, NT), NP = ceil_div(C::ITEMS_P, NT);
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    constexpr int NW = NT / 32;
+    constexpr int NIO = ceil_div(C::ITEMS_IO, NT), NQ = ceil_div(C::ITEMS_Q, 32), NP = ceil_div(C::ITEMS_P, 32);
 
     if (tid == 0) { mbar_init(&full, 1); mbar_fence_init(); }
+    for (int x = tid; x < C::TA; x += NT) {
+        const double2 v = g.twa[x];
+        TW1[x] = v;
+        TW2[(x % C::QA) * C::PA + x / C::QA] = v;
+    }
     __syncthreads();
-    auto block_ptr = [&](int id) -> double2* {             // id -> (t, pch, q), q fastest
-        const int q = id % C::R1, rest = id / C::R1;
-        const int pch = rest % g.npch, t = rest / g.npch;
+    auto block_ptr = [&](int id) -> double2* {             // id -> (pch, q, t), t fastest
+        const int t = id % g.count, rest = id / g.count;
+        const int q = rest % C::R1, pch = rest / C::R1;
         return g.w1 + ((static_cast<size_t>(t) * C::R1 + q) * g.npch + pch) * C::BLOCK_ELEMS;
     };
     auto issue_block_load = [&](int id) {                  // all lanes of warp 0
         const double2* src = block_ptr(id);
         if (tid == 0) mbar_arrive_expect_tx(&full, C::NA * C::ROW_BYTES);
         __syncwarp();
-        for (int a = tid; a < C::NA; a += 32) bulk_g2s(L + a * C::RS, src + a * C::COLS, C::ROW_BYTES, &full);
+        for (int a = tid; a < C::NA; a += 32) bulk_g2s(L + a * C::RSL, src + a * C::COLS, C::ROW_BYTES, &full);
     };
     if (tid < 32 && static_cast<int>(blockIdx.x) < g.ntiles) issue_block_load(blockIdx.x);
 
-    IoIdx io[NIO];
-#pragma unroll
-    for (int m = 0; m < NIO; ++m) io[m] = io_index<C>(tid + m * NT < C::ITEMS_IO ? tid + m * NT : 0);
-    ColAIdx cq[NQ];
-#pragma unroll
-    for (int m = 0; m < NQ; ++m) cq[m] = colq_index<C>(tid + m * NT < C::ITEMS_Q ? tid + m * NT : 0);
-    ColAIdx cp[NP];
-#pragma unroll
-    for (int m = 0; m < NP; ++m) cp[m] = colp_index<C>(tid + m * NT < C::ITEMS_P ? tid + m * NT : 0);
-    const size_t kstride = static_cast<size_t>(C::TB / 2 + 1) * g.tc;
-
     int it = 0;
     for (int id = blockIdx.x; id < g.ntiles; id += gridDim.x, ++it) {
-        const int q = id % C::R1, pch = (id / C::R1) % g.npch;
+        const int rest = id / g.count;
+        const int q = rest % C::R1, pch = rest / C::R1;
         double2* blk = block_ptr(id);
         mbar_wait(&full, it & 1);
 #pragma unroll
         for (int m = 0; m < NIO; ++m)
-            if (tid + m * NT < C::ITEMS_IO) b0_compute<C>(L + io[m].s, W + io[m].s);
-        __syncthreads();
-        if (LAND && tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
-#pragma unroll
-        for (int m = 0; m < NQ; ++m)
-            if (tid + m * NT < C::ITEMS_Q) b1_compute<C>(W + cq[m].base, g.twa + cq[m].k);
-        __syncthreads();
-#pragma unroll
-        for (int m = 0; m < NP; ++m)
-            if (tid + m * NT < C::ITEMS_P) {
-                const int r = cp[m].col / C::CHUNK, pin = cp[m].col % C::CHUNK;
-                const int kb = q + C::R1 * r;
-                const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-                b2_compute<C>(W + cp[m].base, g.ks + static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin, kstride,
-                              g.twa + cp[m].k * C::QA, cp[m].k);
+            if (tid + m * NT < C::ITEMS_IO) {
+                const IoIdx x = io_index<C>(tid + m * NT);
+                b0_compute<C>(L + x.l, W + x.s);
             }
         __syncthreads();
+        if (tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
+        for (int cg = wid; cg < C::NGRP; cg += NW) {
 #pragma unroll
-        for (int m = 0; m < NQ; ++m)
-            if (tid + m * NT < C::ITEMS_Q) b3_compute<C>(W + cq[m].base);
+            for (int m = 0; m < NQ; ++m)
+                if (lane + m * 32 < C::ITEMS_Q) {
+                    const ColAIdx x = colq_index<C>(cg, lane + m * 32);
+                    b1_compute<C>(W + x.base, TW1 + x.k, C::QA);
+                }
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < NP; ++m)
+                if (lane + m * 32 < C::ITEMS_P) {
+                    const ColAIdx x = colp_index<C>(cg, lane + m * 32);
+                    const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
+                    const int kb = q + C::R1 * r;
+                    const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
+                    b2_compute<C>(W + x.base, g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA, TW2 + x.k, C::PA, x.k);
+                }
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < NQ; ++m)
+                if (lane + m * 32 < C::ITEMS_Q) b3_compute<C>(W + colq_index<C>(cg, lane + m * 32).base);
+        }
         __syncthreads();
 #pragma unroll
         for (int m = 0; m < NIO; ++m)
-            if (tid + m * NT < C::ITEMS_IO) b4_compute<C>(W + io[m].s, blk + io[m].g);
-        __syncthreads();
-        if (!LAND && tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
+            if (tid + m * NT < C::ITEMS_IO) {
+                const IoIdx x = io_index<C>(tid + m * NT);
+                b4_compute<C>(W + x.s, blk + x.g);
+            }
     }
 }
 

@@ -15,7 +15,7 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
                      const double2* twa, const double2* twc, const double2* rootsb, const double* ks_sym,
                      double* e_out /*[count][2]*/) {
     using AC = CfgAC<TC, TB, FREE, G, CHUNK>;
-    static_assert(CHUNK == 2 || CHUNK == 4, "chunk");
+    static_assert(CHUNK == 1 || CHUNK == 2 || CHUNK == 4, "chunk");
     using B = CfgB<TA, TB, FREE, CHUNK>;
     const int na = B::NA;
     const long long m_points = static_cast<long long>(na) * AC::NB * AC::NC;
@@ -26,12 +26,15 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
     for (int b2 = 0; b2 < AC::R2; ++b2)
         for (int q = 0; q < AC::R1; ++q) twb[b2 * AC::R1 + q] = rootsb[(b2 * q) % TB];
     const int nah = TA / 2 + 1, nbh = TB / 2 + 1, nch = TC / 2 + 1;
-    std::vector<double> ks(static_cast<size_t>(nah) * nbh * TC);
-    for (int r = 0; r < nah * nbh; ++r)
-        for (int p = 0; p < TC; ++p) {
-            const int kc = (p / AC::QC) + AC::PC * (p % AC::QC);
-            ks[static_cast<size_t>(r) * TC + p] = ks_sym[static_cast<size_t>(r) * nch + (kc <= TC - kc ? kc : TC - kc)];
-        }
+    std::vector<double> ks(static_cast<size_t>(nbh) * TC * nah);      // [sb][p][sa], p = scrambled c position
+    for (int sa = 0; sa < nah; ++sa)
+        for (int sb = 0; sb < nbh; ++sb)
+            for (int p = 0; p < TC; ++p) {
+                const int kc = (p / AC::QC) + AC::PC * (p % AC::QC);
+                ks[(static_cast<size_t>(sb) * TC + p) * nah + sa] = ks_sym[(static_cast<size_t>(sa) * nbh + sb) * nch + (kc <= TC - kc ? kc : TC - kc)];
+            }
+    std::vector<double2> twa2(TA);                                     // [n2*PA + k1]: the kernel's second smem copy
+    for (int x = 0; x < TA; ++x) twa2[(x % B::QA) * B::PA + x / B::QA] = twa[x];
     ArgsAC g{};
     g.psi = psi; g.kpsi = kpsi; g.w1 = w1.data(); g.desc = desc; g.twc = twc; g.twb = twb.data();
     g.m_points = m_points; g.na = na; g.i = i; g.fi = fi; g.count = count;
@@ -68,23 +71,24 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
             }
         }
     }
-    // pass B
+    // pass B (block order and item -> thread mapping differ from the kernel; the index functions are the same)
     const int npch = TC / CHUNK;
-    const size_t kstride = static_cast<size_t>(nbh) * TC;
     for (int id = 0; id < count * B::R1 * npch; ++id) {
         const int q = id % B::R1, pch = (id / B::R1) % npch, t = id / (B::R1 * npch);
         double2* blk = w1.data() + ((static_cast<size_t>(t) * B::R1 + q) * npch + pch) * B::BLOCK_ELEMS;
-        for (int a = 0; a < B::NA; ++a) std::memcpy(&L[a * B::RS], blk + a * B::COLS, B::ROW_BYTES);   // TMA bulk row loads
-        for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b0_compute<B>(L.data() + x.s, W.data() + x.s); }
-        for (int w = 0; w < B::ITEMS_Q; ++w) { const ColAIdx x = colq_index<B>(w); b1_compute<B>(W.data() + x.base, twa + x.k); }
-        for (int w = 0; w < B::ITEMS_P; ++w) {
-            const ColAIdx x = colp_index<B>(w);
-            const int r = x.col / CHUNK, pin = x.col % CHUNK;
-            const int kb = q + B::R1 * r;
-            const int sb = kb <= TB - kb ? kb : TB - kb;
-            b2_compute<B>(W.data() + x.base, ks.data() + static_cast<size_t>(sb) * TC + pch * CHUNK + pin, kstride, twa + x.k * B::QA, x.k);
+        for (int a = 0; a < B::NA; ++a) std::memcpy(&L[a * B::RSL], blk + a * B::COLS, B::ROW_BYTES);   // TMA bulk row loads
+        for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b0_compute<B>(L.data() + x.l, W.data() + x.s); }
+        for (int cg = 0; cg < B::NGRP; ++cg) {
+            for (int w = 0; w < B::ITEMS_Q; ++w) { const ColAIdx x = colq_index<B>(cg, w); b1_compute<B>(W.data() + x.base, twa + x.k, B::QA); }
+            for (int w = 0; w < B::ITEMS_P; ++w) {
+                const ColAIdx x = colp_index<B>(cg, w);
+                const int r = x.col / CHUNK, pin = x.col % CHUNK;
+                const int kb = q + B::R1 * r;
+                const int sb = kb <= TB - kb ? kb : TB - kb;
+                b2_compute<B>(W.data() + x.base, ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, twa2.data() + x.k, B::PA, x.k);
+            }
+            for (int w = 0; w < B::ITEMS_Q; ++w) b3_compute<B>(W.data() + colq_index<B>(cg, w).base);
         }
-        for (int w = 0; w < B::ITEMS_Q; ++w) b3_compute<B>(W.data() + colq_index<B>(w).base);
         for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b4_compute<B>(W.data() + x.s, blk + x.g); }
     }
     // pass C: the W1 columns land in place in the work buffer (the kernel's cp.async gather), psi_j / psi_l lines are
