@@ -13,7 +13,7 @@ LIB = os.path.join(HERE, "libexx_b200.so")
 SOURCES = ["exx_api.cu", "exx_pass_a.cu", "exx_pass_b.cu", "exx_pass_c.cu"]
 HEADERS = ["exx_dft.cuh", "exx_passes.cuh", "exx_launch.h", "exx_inst.cuh", "exx_sched.hpp", "../../include/exx.h"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC"]
+FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-Xcompiler", "-fPIC"] + os.environ.get("EXX_EXTRA_NVCC_FLAGS", "").split()
 
 
 def _nvcc() -> str:

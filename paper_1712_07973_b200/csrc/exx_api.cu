@@ -1,6 +1,6 @@
 // exx_api.cu -- plan, tables, pair scheduling and the C ABI of libexx_b200 (include/exx.h).
 //
-// Hot path per same-i batch (PAPER.md:113-117 kernels 1-3, fused): pass A -> pass B -> pass C -> energy reduce,
+// Hot path per same-(j,l) batch (PAPER.md:113-117 kernels 1-3, fused): pass A -> pass B -> pass C -> energy reduce,
 // all enqueued on the plan's stream; the host only schedules.  No CPU fallback exists anywhere in this file:
 // without a usable CUDA device every computing entry point returns EXX_ERR_CUDA.
 #include <cmath>
@@ -97,7 +97,7 @@ __global__ void permute_kernel_axes(const double* ks_sym, double* ks_perm, int n
 }
 
 // e_ij = dV * sum over tiles of the per-CTA partial sums of pass C, fixed order (deterministic).
-__global__ void reduce_energy_kernel(const double* epart, int tiles, const XformDesc* desc, int i, int n_orb, double dV,
+__global__ void reduce_energy_kernel(const double* epart, int tiles, const XformDesc* desc, int j, int l, int n_orb, double dV,
                                      double* e_mat) {
     __shared__ double sh[2][256];
     const int t = blockIdx.x;
@@ -112,13 +112,15 @@ __global__ void reduce_energy_kernel(const double* epart, int tiles, const Xform
     }
     if (threadIdx.x == 0) {
         const XformDesc d = desc[t];
-        const double e1 = dV * sh[0][0];
-        e_mat[static_cast<size_t>(i) * n_orb + d.j] = e1;
-        e_mat[static_cast<size_t>(d.j) * n_orb + i] = e1;
-        if (d.l >= 0) {
+        if (d.flags & 1) {
+            const double e1 = dV * sh[0][0];
+            e_mat[static_cast<size_t>(j) * n_orb + d.i] = e1;
+            e_mat[static_cast<size_t>(d.i) * n_orb + j] = e1;
+        }
+        if (d.flags & 2) {
             const double e2 = dV * sh[1][0];
-            e_mat[static_cast<size_t>(i) * n_orb + d.l] = e2;
-            e_mat[static_cast<size_t>(d.l) * n_orb + i] = e2;
+            e_mat[static_cast<size_t>(l) * n_orb + d.i] = e2;
+            e_mat[static_cast<size_t>(d.i) * n_orb + l] = e2;
         }
     }
 }
@@ -388,7 +390,7 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
     };
     for (const Batch& b : sched.batches) {
         ac.desc = p->desc_dev + b.first;
-        ac.i = b.i; ac.fi = occ_host[b.i]; ac.count = b.count;
+        ac.j = b.j; ac.l = b.l; ac.fj = b.fj; ac.fl = b.fl; ac.count = b.count;
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_a(p->geo, ac, s, nullptr));
         EXX_CUDA(p, mark());
@@ -396,7 +398,7 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
         EXX_CUDA(p, mark());
-        reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_c.tiles, ac.desc, b.i, n_orb, p->dV, p->e_mat);
+        reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_c.tiles, ac.desc, b.j, b.l, n_orb, p->dV, p->e_mat);
         EXX_CUDA(p, cudaGetLastError());
         EXX_CUDA(p, mark());
         p->launches += 4;

@@ -46,13 +46,14 @@ constexpr int imax(int a, int b) { return a > b ? a : b; }
 // bytes of dynamic shared memory of pass A (one work buffer) / pass C (two work buffers, R1 lines per b2) for a tile of
 // g b2-values with `nstg` operand stages (mirrors CfgAC)
 template <int TC, int TB, bool FREE>
-constexpr int smem_ac_bytes(int g, int nstg, bool pass_c) {
+constexpr int smem_ac_bytes(int g, int nstg, bool pass_c, int nbuf = 2) {
     constexpr int PC = Split<TC>::P, QC = Split<TC>::Q, R1 = BSplit<TB>::R1;
     constexpr int NB1 = FREE ? R1 / 2 : R1, NC = FREE ? TC / 2 : TC;
     constexpr int ROW = PC * (QC | 1);
     constexpr int LS = NC + (((QC - NC % 16) % 16) + 16) % 16;
     const int work = g * ((pass_c ? R1 : NB1) * ROW + (g > 1 ? 4 : 0)) * 16;
-    return (pass_c ? 2 : 1) * work + nstg * 2 * g * NB1 * LS * 8;
+    const int lines = g * NB1 * LS * 8;                    // one orbital's lines of the tile
+    return (pass_c ? nbuf : 1) * work + nstg * lines + (pass_c ? 2 * lines : 0);
 }
 
 // largest G dividing R2 with at most 256 (line, n2) items per tile whose tile fits shared memory
@@ -66,9 +67,18 @@ constexpr int pick_g(bool pass_c, int max_bytes) {
     return g;
 }
 
-// resident CTAs per SM to compile for: limited by shared memory, by a register floor per thread, and by `cap`
-constexpr int pick_minb(int smem, int nt, int reg_floor, int cap) {
-    return imax(1, imin(imin(kSmemPerSM / (smem + 1024), 65536 / (nt * reg_floor)), cap));
+// resident CTAs per SM to compile for: limited by shared memory, by a register floor per thread, and by `cap`; among
+// the admissible counts the one that wastes the fewest CTA slots in the last wave of a cubic grid's `tiles` CTAs on 148
+// SMs wins (a tile is a long loop over the batch, so a ragged last wave costs a whole loop), ties -> more CTAs
+constexpr int pick_minb(int smem, int nt, int reg_floor, int cap, int tiles) {
+    const int maxb = imax(1, imin(imin(kSmemPerSM / (smem + 1024), 65536 / (nt * reg_floor)), cap));
+    int best = 1, best_eff = -1;
+    for (int b = 1; b <= maxb; ++b) {
+        const int slots = 148 * b, waves = (tiles + slots - 1) / slots;
+        const int eff = tiles * 1000 / (waves * slots) + (b > 1 ? 30 : 0);     // co-residency itself is worth a little
+        if (eff >= best_eff) { best_eff = eff; best = b; }
+    }
+    return best;
 }
 
 template <int TC, int TB, bool FREE>
@@ -78,16 +88,18 @@ struct TuneAC {
     static constexpr int G_C = pick_g<TC, TB, FREE>(true, kMaxSmemAC / 2);
     using CfgC = CfgAC<TC, TB, FREE, G_C, CHUNK>;
     static constexpr int NT_C = imax(32, round_up32(imax(CfgC::ITEMS_LINE_Q, imin(CfgC::ITEMS_POS, 256))));
-    static constexpr int NSTG_C = smem_ac_bytes<TC, TB, FREE>(G_C, 2, true) <= kMaxSmemAC ? 2 : 1;
-    static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true);
-    static constexpr int MINB_C = pick_minb(SMEM_C, NT_C, 128, 4);
+    // double-buffered W1 tile where it fits next to one operand stage and the resident lines, else single-buffered
+    static constexpr int NBUF_C = smem_ac_bytes<TC, TB, FREE>(G_C, 1, true, 2) <= kMaxSmemAC ? 2 : 1;
+    static constexpr int NSTG_C = smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, NBUF_C) <= kMaxSmemAC ? 2 : 1;
+    static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true, NBUF_C);
+    static constexpr int MINB_C = pick_minb(SMEM_C, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A
     static constexpr int G_A = pick_g<TC, TB, FREE>(false, kMaxSmemAC / 3);
     using CfgA = CfgAC<TC, TB, FREE, G_A, CHUNK>;
     static constexpr int NT_A = imax(32, round_up32(imax(CfgA::ITEMS_LINE_Q, imin(CfgA::ITEMS_POS, 256))));
     static constexpr int NSTG_A = 2;
     static constexpr int SMEM_A = smem_ac_bytes<TC, TB, FREE>(G_A, NSTG_A, false);
-    static constexpr int MINB_A = pick_minb(SMEM_A, NT_A, 96, 4);
+    static constexpr int MINB_A = pick_minb(SMEM_A, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
     static_assert(SMEM_C <= kMaxSmemAC && SMEM_A <= kMaxSmemAC, "tile does not fit shared memory");
 };
 

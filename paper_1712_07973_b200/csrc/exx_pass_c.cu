@@ -21,8 +21,8 @@ static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     using T = TuneAC<TC, TB, FREE>;
     using C = typename T::CfgC;
     constexpr int smem = T::SMEM_C;
-    static_assert(smem == 2 * C::SMEM_C * 16 + T::NSTG_C * C::OP_DOUBLES * 8, "pass C shared memory");
-    auto kern = pass_c_kernel<C, T::NT_C, T::NSTG_C, T::MINB_C>;
+    static_assert(smem == T::NBUF_C * C::SMEM_C * 16 + (T::NSTG_C * C::OP_DOUBLES + C::RES_DOUBLES) * 8, "pass C shared memory");
+    auto kern = pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C>;
     static bool done = false;
     static int occ = 0;
     if (info) { info->threads = T::NT_C; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }

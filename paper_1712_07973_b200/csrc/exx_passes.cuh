@@ -65,10 +65,12 @@ constexpr int split_p(int t) { return t == 16 ? 4 : t == 32 ? 4 : t == 64 ? 8 : 
 constexpr int split_q(int t) { return t / split_p(t); }
 constexpr int chunk_for(int ta, int tb, bool free_bc);     // defined after the pass-B geometry helpers
 
-// One packed transform of a same-i batch: pairs (i,j) and (i,l); l < 0 = the imaginary slot is empty.
+// One packed transform of a same-(j,l) batch: the streamed orbital i forms the pairs (j,i) [real part] and (l,i)
+// [imaginary part] with the two resident orbitals of the batch.
 struct XformDesc {
-    int j, l;
-    double fj, fl;
+    int i;
+    int flags;                  // bit 0: pair (j,i) present, bit 1: pair (l,i) present
+    double fi;
 };
 
 EXX_HD double2 ld_ro(const double2* p) {
@@ -126,10 +128,11 @@ struct CfgAC {
     static constexpr int SMEM_A = G * GSTR_A;
     static constexpr int GSTR_C = R1 * ROW + GPAD;         // pass C: the W1 tile lands in place, R1 lines per gi
     static constexpr int SMEM_C = G * GSTR_C;
-    // operand lines (psi_j, psi_l; pass C overwrites them with the K psi_j, K psi_l increments) staged in shared
-    // memory: line stride LS doubles, LS = QC (mod 16) keeps the (line, n2)-mapped 8-byte accesses conflict-free
+    // operand lines (the streamed psi_i; pass C overwrites them with the K psi_i increment) staged in shared memory:
+    // line stride LS doubles, LS = QC (mod 16) keeps the (line, n2)-mapped 8-byte accesses conflict-free
     static constexpr int LS = NC + (((QC - NC % 16) % 16) + 16) % 16;
-    static constexpr int OP_DOUBLES = 2 * LINES * LS;      // one stage: [slot j|l][line][LS]
+    static constexpr int OP_DOUBLES = LINES * LS;          // one stage: [line][LS]
+    static constexpr int RES_DOUBLES = 2 * LINES * LS;     // pass C: the resident psi_j, psi_l lines [slot j|l][line][LS]
     static constexpr int LINE_BYTES = NC * 8;
     static_assert(LS % 2 == 0 && NC % 2 == 0, "16-byte alignment of operand lines");
     // W1 strides in elements ([t][q][pch][a][b2][pin], na = grid points along a)
@@ -150,8 +153,8 @@ struct ArgsAC {
     double* epart;              // pass C: [count][ntiles][2] partial sums of rho*V
     long long m_points;         // na*nb*nc
     int na;
-    int i;                      // common orbital of the batch
-    double fi;
+    int j, l;                   // resident orbitals of the batch (l < 0: none; the imaginary slot is then never present)
+    double fj, fl;
     int count;                  // transforms in the batch
 };
 
@@ -205,16 +208,22 @@ EXX_HD ColIdx col_index(int w, int a, int b2base, int na) {
 }
 
 // ---------------------------------------------------------------------------------------- pass A phases
-// ---- A0: co-density (Eq. 8) + zero padding + stage 1 of the c-axis FFT.
-//      vi = psi_i at the item's PCN points; pj / pl = psi_j / psi_l at the item's first point, stride QC doubles
-//      between the points; row = work-buffer row of the item; tw = twc + n2.
+// ---- A0: co-densities (Eq. 8) z = psi_i psi_j + i psi_i psi_l + zero padding + stage 1 of the c-axis FFT.
+//      vj / vl = psi_j / psi_l at the item's PCN points (registers); pi = the streamed psi_i at the item's first point,
+//      stride QC doubles between the points; row = work-buffer row of the item; tw = twc + n2.
 template <class C>
-EXX_HD void a0_compute(const double* vi, const double* pj, const double* pl, double lmask, double2* row, const double2* tw) {
+EXX_HD void a0_compute(const double* vj, const double* vl, const double* pi, int flags, double2* row, const double2* tw) {
     double xr[C::PC], xi[C::PC];
 #pragma unroll
     for (int n1 = 0; n1 < C::PCN; ++n1) {
-        xr[n1] = vi[n1] * pj[C::QC * n1];
-        xi[n1] = vi[n1] * pl[C::QC * n1] * lmask;
+        const double p = pi[C::QC * n1];
+        xr[n1] = vj[n1] * p;
+        xi[n1] = vl[n1] * p;
+    }
+    if (flags != 3) {                                          // an absent pair contributes an exactly zero co-density
+        const double m1 = (flags & 1) ? 1.0 : 0.0, m2 = (flags & 2) ? 1.0 : 0.0;
+#pragma unroll
+        for (int n1 = 0; n1 < C::PCN; ++n1) { xr[n1] *= m1; xi[n1] *= m2; }
     }
 #pragma unroll
     for (int n1 = C::PCN; n1 < C::PC; ++n1) { xr[n1] = 0.0; xi[n1] = 0.0; }
@@ -285,34 +294,37 @@ EXX_HD void c1_compute(double2* seg, const double2* tw, int k1) {
 }
 
 // ---- C2: inverse stage over k1 (P-point) of the c axis, then "Kernel 3" for the PCN points
-//      c = QC n1 + n2 of the line that this item owns:
-//      acc   += f_j V_ij psi_j + f_l V_il psi_l                 (K psi_i -= acc after the batch)
-//      oj    <- -f_i V_ij psi_i ,  ol <- -f_i V_il psi_i         increments of K psi_j, K psi_l, written over the
-//               staged psi_j / psi_l values and added to K psi by the memory system   PAPER.md:67-69 Eq. 3, :111
-//      e1    += rho_ij V_ij,  e2 += rho_il V_il                                        PAPER.md:81-82 Eq. 5
-//      vi = psi_i at the item's points; oj / ol = operand lines at the item's first point (stride QC doubles).
+//      c = QC n1 + n2 of the line that this item owns, with V1 = V_ji = Re, V2 = V_li = Im:
+//      accj  += f_i V1 psi_i ,  accl += f_i V2 psi_i            (K psi_j -= accj, K psi_l -= accl after the batch)
+//      oi    <- -(f_j V1 psi_j + f_l V2 psi_l)                   increment of K psi_i, written over the staged psi_i
+//               values and added to K psi_i by the memory system          PAPER.md:67-69 Eq. 3, :111
+//      e1    += rho_ji V1,  e2 += rho_li V2                                         PAPER.md:81-82 Eq. 5
+//      i == j (diagonal pair (j,j), imaginary slot absent) and i == l (pairs (j,l) and (l,l)) produce no increment
+//      of K psi_i: the cross term f_j V_jl psi_j of K psi_l goes into accl instead, so every K psi address receives
+//      exactly one reduce-add per launch.
+//      rj / rl = resident psi_j / psi_l lines, oi = operand line, all at the item's first point (stride QC doubles).
 template <class C>
-EXX_HD void c2_compute(const double2* row, const XformDesc& d, double fi, const double* vi /*[PCN]*/, double* oj,
-                       double* ol, double* acc /*[PCN]*/, double& e1, double& e2) {
+EXX_HD void c2_compute(const double2* row, const XformDesc& d, int l, double fj, double fl, const double* rj, const double* rl,
+                       double* oi, double* accj /*[PCN]*/, double* accl /*[PCN]*/, double& e1, double& e2) {
     double xr[C::PC], xi[C::PC];
 #pragma unroll
     for (int k1 = 0; k1 < C::PC; ++k1) { double2 v = row[k1 * C::QCP]; xr[k1] = v.x; xi[k1] = v.y; }
     dft_inv<C::PC, C::FREE>(xr, xi);
-    const bool has_l = d.l >= 0;
-    const double fl = has_l ? d.fl : 0.0;
+    const double m1 = (d.flags & 1) ? 1.0 : 0.0, m2 = (d.flags & 2) ? 1.0 : 0.0;
+    const double fjl = d.i == l ? fj : 0.0;
     double s1 = 0.0, s2 = 0.0;
 #pragma unroll
     for (int n1 = 0; n1 < C::PCN; ++n1) {
         const int off = C::QC * n1;
-        const double v1 = xr[n1], v2 = xi[n1];
-        const double vj = oj[off];
-        const double vl = has_l ? ol[off] : 0.0;
-        const double a1 = v1 * vi[n1], a2 = v2 * vi[n1];     // V_ij psi_i, V_il psi_i
-        acc[n1] += d.fj * (v1 * vj) + fl * (v2 * vl);
-        oj[off] = -(fi * a1);
-        if (has_l) ol[off] = -(fi * a2);
-        s1 += a1 * vj;
-        s2 += a2 * vl;
+        const double v1 = xr[n1] * m1, v2 = xi[n1] * m2;
+        const double pi = oi[off], pj = rj[off], pl = rl[off];
+        const double a1 = v1 * pi, a2 = v2 * pi;              // V_ji psi_i, V_li psi_i
+        const double b1 = v1 * pj, b2 = v2 * pl;              // V_ji psi_j, V_li psi_l
+        accj[n1] += d.fi * a1;
+        accl[n1] += d.fi * a2 + fjl * b1;
+        oi[off] = -(fj * b1 + fl * b2);
+        s1 += a1 * pj;
+        s2 += a2 * pl;
     }
     e1 += s1;
     e2 += s2;
@@ -555,22 +567,24 @@ EXX_HD void b4_compute(const double2* src, double2* dst) {
 
 __host__ __device__ constexpr int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
-// TMA bulk loads of the psi_j / psi_l lines of one transform into an operand stage (all 32 lanes of warp 0 call this)
+// TMA bulk loads of the LINES lines of orbital `orb` of tile (a, b2base) into [line][LS] shared memory; the caller has
+// armed `bar` with the byte count (all 32 lanes of one warp call this)
+template <class C>
+__device__ __forceinline__ void issue_line_loads(const ArgsAC& g, int orb, double* dst, uint64_t* bar, int a, int b2base, int lane) {
+    const double* base = g.psi + static_cast<size_t>(orb) * g.m_points;
+    for (int l = lane; l < C::LINES; l += 32) bulk_g2s(dst + l * C::LS, base + line_offset<C>(l, a, b2base), C::LINE_BYTES, bar);
+}
+// the streamed psi_i lines of one transform into an operand stage
 template <class C>
 __device__ __forceinline__ void issue_operand_loads(const ArgsAC& g, const XformDesc& d, double* stage, uint64_t* bar, int a,
                                                     int b2base, int lane) {
-    const int nops = (d.l >= 0 ? 2 : 1) * C::LINES;
-    if (lane == 0) mbar_arrive_expect_tx(bar, nops * C::LINE_BYTES);
+    if (lane == 0) mbar_arrive_expect_tx(bar, C::LINES * C::LINE_BYTES);
     __syncwarp();
-    for (int o = lane; o < nops; o += 32) {
-        const int slot = o / C::LINES, l = o % C::LINES;
-        const double* src = g.psi + static_cast<size_t>(slot ? d.l : d.j) * g.m_points + line_offset<C>(l, a, b2base);
-        bulk_g2s(stage + (slot * C::LINES + l) * C::LS, src, C::LINE_BYTES, bar);
-    }
+    issue_line_loads<C>(g, d.i, stage, bar, a, b2base, lane);
 }
 
-// Pass A.  One CTA per (a, b2-group) tile, looping over the transforms of the same-i batch.  psi_i of the thread's
-// points lives in registers; psi_j / psi_l lines arrive NSTG transforms ahead by TMA bulk copies.
+// Pass A.  One CTA per (a, b2-group) tile, looping over the transforms of the same-(j,l) batch.  psi_j and psi_l of the
+// thread's points live in registers; the streamed psi_i lines arrive NSTG transforms ahead by TMA bulk copies.
 template <class C, int NT, int NSTG, int MINB>
 __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -592,14 +606,15 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
 
     // per-thread items, resolved once
     LineQIdx q0[NI0];
-    double vi[NI0][C::PCN];
+    double vj[NI0][C::PCN], vl[NI0][C::PCN];
 #pragma unroll
     for (int m = 0; m < NI0; ++m) {
         const int w = tid + m * NT;
         q0[m] = lineq_index<C, false>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
-        const double* pi = g.psi + static_cast<size_t>(g.i) * g.m_points + q0[m].gofs;
+        const double* pj = g.psi + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
+        const double* pl = g.psi + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
 #pragma unroll
-        for (int n1 = 0; n1 < C::PCN; ++n1) vi[m][n1] = ld_ro(pi + C::QC * n1);
+        for (int n1 = 0; n1 < C::PCN; ++n1) { vj[m][n1] = ld_ro(pj + C::QC * n1); vl[m][n1] = ld_ro(pl + C::QC * n1); }
     }
     LinePIdx p1[NI1];
 #pragma unroll
@@ -612,14 +627,12 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     for (int t = 0; t < g.count; ++t) {
         const int s = t % NSTG;
         double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
-        const XformDesc d = g.desc[t];
-        const double lmask = d.l < 0 ? 0.0 : 1.0;
-        const int lofs = d.l < 0 ? 0 : C::LINES * C::LS;       // empty imaginary slot: read psi_j, multiply by 0
+        const int flags = g.desc[t].flags;
         mbar_wait(&full[s], (t / NSTG) & 1);
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
             if (tid + m * NT < C::ITEMS_LINE_Q)
-                a0_compute<C>(vi[m], stage + q0[m].op, stage + lofs + q0[m].op, lmask, S + q0[m].row, g.twc + q0[m].n2);
+                a0_compute<C>(vj[m], vl[m], stage + q0[m].op, flags, S + q0[m].row, g.twc + q0[m].n2);
         __syncthreads();
         if (tid < 32 && t + NSTG < g.count)                    // the stage has been consumed: refill it
             issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
@@ -719,19 +732,23 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
     }
 }
 
-// Pass C.  One CTA per (a, b2-group) tile; it loops over the transforms of the same-i batch, keeps the K psi_i
-// accumulator and psi_i of its points in registers, and is software-pipelined:
+// Pass C.  One CTA per (a, b2-group) tile; it loops over the transforms of the same-(j,l) batch, keeps the K psi_j and
+// K psi_l accumulators of its points in registers and the psi_j / psi_l lines of the tile resident in shared memory,
+// and is software-pipelined:
 //   * every thread gathers the W1 columns it will transform (C0) for transform t+1 into the second work buffer with
 //     16-byte cp.async while t is computed (128-byte runs, see col_index);
-//   * psi_j / psi_l lines arrive NSTG transforms ahead by TMA bulk copies (mbarrier completion) into operand stages;
-//   * the K psi_j / K psi_l increments overwrite those lines and leave by TMA bulk reduce-add (fp64) -- each K psi
-//     address receives exactly one add per launch (the j of a batch are distinct), so the result is deterministic.
-template <class C, int NT, int NSTG, int MINB>
+//   * the streamed psi_i lines arrive NSTG transforms ahead by TMA bulk copies (mbarrier completion) into operand stages;
+//   * the K psi_i increment overwrites those lines and leaves by TMA bulk reduce-add (fp64) -- each K psi address
+//     receives exactly one add per launch (the i of a batch are distinct and never j or l), so the result is
+//     deterministic.
+template <class C, int NT, int NSTG, int NBUF, int MINB>
 __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* const S0 = reinterpret_cast<double2*>(smem_raw);
-    double* const OP = reinterpret_cast<double*>(S0 + 2 * C::SMEM_C);
+    double* const OP = reinterpret_cast<double*>(S0 + NBUF * C::SMEM_C);
+    double* const RES = OP + NSTG * C::OP_DOUBLES;
     __shared__ uint64_t full[NSTG];
+    __shared__ uint64_t resbar;
     __shared__ double red[2][NT / 32];
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
@@ -739,6 +756,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
 
     if (tid == 0) {
         for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
+        mbar_init(&resbar, 1);
         mbar_fence_init();
     }
     __syncthreads();
@@ -748,7 +766,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     for (int m = 0; m < NI0; ++m) c0[m] = col_index<C, true>(tid + m * NT < C::ITEMS_POS ? tid + m * NT : 0, a, b2base, g.na);
     const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
     auto issue_w1_gather = [&](int t) {
-        double2* dstbuf = S0 + (t & 1) * C::SMEM_C;
+        double2* dstbuf = S0 + (NBUF == 2 ? (t & 1) : 0) * C::SMEM_C;
         const double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
@@ -757,34 +775,46 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
                 for (int q = 0; q < C::R1; ++q) cp_async16(dstbuf + c0[m].col + q * C::ROW, w1t + c0[m].w1 + q * qstride);
             }
     };
-    issue_w1_gather(0);
-    cp_async_commit();
-    if (tid < 32)
+    if (NBUF == 2) {
+        issue_w1_gather(0);
+        cp_async_commit();
+    }
+    if (tid < 32) {
+        if (tid == 0) mbar_arrive_expect_tx(&resbar, 2 * C::LINES * C::LINE_BYTES);
+        __syncwarp();
+        issue_line_loads<C>(g, g.j, RES, &resbar, a, b2base, tid);
+        issue_line_loads<C>(g, g.l >= 0 ? g.l : g.j, RES + C::LINES * C::LS, &resbar, a, b2base, tid);
         for (int t = 0; t < NSTG && t < g.count; ++t)
             issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+    }
 
     LinePIdx p1[NI1];
 #pragma unroll
     for (int m = 0; m < NI1; ++m) p1[m] = linep_index<C, true>(tid + m * NT < C::ITEMS_LINE_P ? tid + m * NT : 0);
     LineQIdx q2[NI2];
-    double vi[NI2][C::PCN], acc[NI2][C::PCN];
+    double accj[NI2][C::PCN], accl[NI2][C::PCN];
 #pragma unroll
     for (int m = 0; m < NI2; ++m) {
         const int w = tid + m * NT;
         q2[m] = lineq_index<C, true>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
-        const double* pi = g.psi + static_cast<size_t>(g.i) * g.m_points + q2[m].gofs;
 #pragma unroll
-        for (int n1 = 0; n1 < C::PCN; ++n1) { vi[m][n1] = ld_ro(pi + C::QC * n1); acc[m][n1] = 0.0; }
+        for (int n1 = 0; n1 < C::PCN; ++n1) { accj[m][n1] = 0.0; accl[m][n1] = 0.0; }
     }
 
     for (int t = 0; t < g.count; ++t) {
-        double2* S = S0 + (t & 1) * C::SMEM_C;
+        double2* S = S0 + (NBUF == 2 ? (t & 1) : 0) * C::SMEM_C;
         const int s = t % NSTG;
         double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
         const XformDesc d = g.desc[t];
-        if (t + 1 < g.count) issue_w1_gather(t + 1);
-        cp_async_commit();
-        cp_async_wait<1>();                                // this thread's columns of transform t have landed
+        if (NBUF == 2) {
+            if (t + 1 < g.count) issue_w1_gather(t + 1);
+            cp_async_commit();
+            cp_async_wait<1>();                            // this thread's columns of transform t have landed
+        } else {                                           // single work buffer: no overlap of the gather
+            issue_w1_gather(t);
+            cp_async_commit();
+            cp_async_wait<0>();
+        }
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
             if (tid + m * NT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, g.twb + c0[m].b2 * C::R1);
@@ -793,12 +823,14 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         for (int m = 0; m < NI1; ++m)
             if (tid + m * NT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, g.twc + p1[m].k1 * C::QC, p1[m].k1);
         __syncthreads();
-        mbar_wait(&full[s], (t / NSTG) & 1);               // psi_j / psi_l lines of transform t have landed
+        if (t == 0) mbar_wait(&resbar, 0);                 // psi_j / psi_l lines of the tile
+        mbar_wait(&full[s], (t / NSTG) & 1);               // psi_i lines of transform t have landed
         double e1 = 0.0, e2 = 0.0;
 #pragma unroll
         for (int m = 0; m < NI2; ++m)
             if (tid + m * NT < C::ITEMS_LINE_Q)
-                c2_compute<C>(S + q2[m].row, d, g.fi, vi[m], stage + q2[m].op, stage + C::LINES * C::LS + q2[m].op, acc[m], e1, e2);
+                c2_compute<C>(S + q2[m].row, d, g.l, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                              accj[m], accl[m], e1, e2);
         fence_proxy_async();                               // increments visible to the TMA reads below
         // block reduction of the energy partials in a fixed order (deterministic)
 #pragma unroll
@@ -816,13 +848,11 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             ep[0] = s1; ep[1] = s2;
         }
         if (tid < 32) {
-            // K psi_j += -f_i V_ij psi_i,  K psi_l += -f_i V_il psi_i   (the same V_ij serves both orbitals)
-            const bool upd_j = d.j != g.i, upd_l = d.l >= 0 && d.l != g.i;
-            for (int o = tid; o < 2 * C::LINES; o += 32) {
-                const int slot = o / C::LINES, l = o % C::LINES;
-                if (slot ? upd_l : upd_j)
-                    bulk_red_add_f64(g.kpsi + static_cast<size_t>(slot ? d.l : d.j) * g.m_points + line_offset<C>(l, a, b2base),
-                                     stage + (slot * C::LINES + l) * C::LS, C::LINE_BYTES);
+            // K psi_i += -(f_j V_ji psi_j + f_l V_li psi_l)   (the same V serves both orbitals of a pair)
+            if (d.flags != 0 && d.i != g.j && d.i != g.l) {
+                double* ki = g.kpsi + static_cast<size_t>(d.i) * g.m_points;
+                for (int l = tid; l < C::LINES; l += 32)
+                    bulk_red_add_f64(ki + line_offset<C>(l, a, b2base), stage + l * C::LS, C::LINE_BYTES);
             }
             bulk_commit();
             if (t + NSTG < g.count) {
@@ -832,13 +862,18 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             }
         }
     }
-    // K psi_i -= sum over the batch (this CTA is the only writer of its tile of K psi_i in this launch)
+    // K psi_j -= accj, K psi_l -= accl (this CTA is the only writer of its tile of K psi_j, K psi_l in this launch)
 #pragma unroll
     for (int m = 0; m < NI2; ++m)
         if (tid + m * NT < C::ITEMS_LINE_Q) {
-            double* ki = g.kpsi + static_cast<size_t>(g.i) * g.m_points + q2[m].gofs;
+            double* kj = g.kpsi + static_cast<size_t>(g.j) * g.m_points + q2[m].gofs;
 #pragma unroll
-            for (int n1 = 0; n1 < C::PCN; ++n1) ki[C::QC * n1] -= acc[m][n1];
+            for (int n1 = 0; n1 < C::PCN; ++n1) kj[C::QC * n1] -= accj[m][n1];
+            if (g.l >= 0) {
+                double* kl = g.kpsi + static_cast<size_t>(g.l) * g.m_points + q2[m].gofs;
+#pragma unroll
+                for (int n1 = 0; n1 < C::PCN; ++n1) kl[C::QC * n1] -= accl[m][n1];
+            }
         }
     if (tid < 32) bulk_wait_read_all();                    // shared memory must outlive the TMA reads
 }

@@ -11,7 +11,7 @@
 using namespace exx;
 
 template <int TA, int TB, int TC, bool FREE, int G, int CHUNK>
-static int emu_batch(const double* psi, double* kpsi, int i, double fi, int count, const XformDesc* desc,
+static int emu_batch(const double* psi, double* kpsi, int j, int l, double fj, double fl, int count, const XformDesc* desc,
                      const double2* twa, const double2* twc, const double2* rootsb, const double* ks_sym,
                      double* e_out /*[count][2]*/) {
     using AC = CfgAC<TC, TB, FREE, G, CHUNK>;
@@ -37,32 +37,32 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
     for (int x = 0; x < TA; ++x) twa2[(x % B::QA) * B::PA + x / B::QA] = twa[x];
     ArgsAC g{};
     g.psi = psi; g.kpsi = kpsi; g.w1 = w1.data(); g.desc = desc; g.twc = twc; g.twb = twb.data();
-    g.m_points = m_points; g.na = na; g.i = i; g.fi = fi; g.count = count;
+    g.m_points = m_points; g.na = na; g.j = j; g.l = l; g.fj = fj; g.fl = fl; g.count = count;
     const size_t qstride = AC::w1_q(na), tstride = AC::w1_t(na);
     std::vector<double2> S(AC::SMEM_A), SC(AC::SMEM_C), W(B::WORK_ELEMS), L(B::LAND_ELEMS);
-    std::vector<double> op(AC::OP_DOUBLES);
-    std::vector<double> vi(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN), acc(vi.size());
-    auto stage_operands = [&](const XformDesc& d, int a, int b2base) {      // the kernels' TMA bulk line loads
-        for (int slot = 0; slot < (d.l >= 0 ? 2 : 1); ++slot)
-            for (int l = 0; l < AC::LINES; ++l)
-                std::memcpy(&op[(slot * AC::LINES + l) * AC::LS],
-                            psi + static_cast<size_t>(slot ? d.l : d.j) * m_points + line_offset<AC>(l, a, b2base), AC::NC * sizeof(double));
+    std::vector<double> op(AC::OP_DOUBLES), res(AC::RES_DOUBLES);
+    std::vector<double> vj(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN), vl(vj.size()), accj(vj.size()), accl(vj.size());
+    auto stage_lines = [&](int orb, double* dst, int a, int b2base) {       // the kernels' TMA bulk line loads
+        for (int ln = 0; ln < AC::LINES; ++ln)
+            std::memcpy(dst + ln * AC::LS, psi + static_cast<size_t>(orb) * m_points + line_offset<AC>(ln, a, b2base), AC::NC * sizeof(double));
     };
+    const int lsafe = l >= 0 ? l : j;
     // pass A
     for (int tile = 0; tile < ntiles; ++tile) {
         const int a = tile / AC::TILES_PER_A, b2base = (tile % AC::TILES_PER_A) * G;
         for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
             const LineQIdx x = lineq_index<AC, false>(w, a, b2base);
-            for (int n1 = 0; n1 < AC::PCN; ++n1) vi[static_cast<size_t>(w) * AC::PCN + n1] = psi[static_cast<size_t>(i) * m_points + x.gofs + AC::QC * n1];
+            for (int n1 = 0; n1 < AC::PCN; ++n1) {
+                vj[static_cast<size_t>(w) * AC::PCN + n1] = psi[static_cast<size_t>(j) * m_points + x.gofs + AC::QC * n1];
+                vl[static_cast<size_t>(w) * AC::PCN + n1] = psi[static_cast<size_t>(lsafe) * m_points + x.gofs + AC::QC * n1];
+            }
         }
         for (int t = 0; t < count; ++t) {
             const XformDesc d = desc[t];
-            stage_operands(d, a, b2base);
-            const double lmask = d.l < 0 ? 0.0 : 1.0;
-            const int lofs = d.l < 0 ? 0 : AC::LINES * AC::LS;
+            stage_lines(d.i, op.data(), a, b2base);
             for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
                 const LineQIdx x = lineq_index<AC, false>(w, a, b2base);
-                a0_compute<AC>(&vi[static_cast<size_t>(w) * AC::PCN], &op[x.op], &op[lofs + x.op], lmask, S.data() + x.row, twc + x.n2);
+                a0_compute<AC>(&vj[static_cast<size_t>(w) * AC::PCN], &vl[static_cast<size_t>(w) * AC::PCN], &op[x.op], d.flags, S.data() + x.row, twc + x.n2);
             }
             for (int w = 0; w < AC::ITEMS_LINE_P; ++w) a1_compute<AC>(S.data() + linep_index<AC, false>(w).seg);
             for (int w = 0; w < AC::ITEMS_POS; ++w) {
@@ -91,16 +91,15 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
         }
         for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b4_compute<B>(W.data() + x.s, blk + x.g); }
     }
-    // pass C: the W1 columns land in place in the work buffer (the kernel's cp.async gather), psi_j / psi_l lines are
-    // staged in an operand buffer that C2 overwrites with the K psi_j / K psi_l increments (the kernel's TMA bulk
-    // loads and bulk reduce-adds are plain copies / adds here).
+    // pass C: the W1 columns land in place in the work buffer (the kernel's cp.async gather); psi_j / psi_l lines are
+    // resident, the psi_i lines are staged in an operand buffer that C2 overwrites with the K psi_i increment (the
+    // kernel's TMA bulk loads and bulk reduce-adds are plain copies / adds here).
     for (int tile = 0; tile < ntiles; ++tile) {
         const int a = tile / AC::TILES_PER_A, b2base = (tile % AC::TILES_PER_A) * G;
-        std::fill(acc.begin(), acc.end(), 0.0);
-        for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
-            const LineQIdx x = lineq_index<AC, true>(w, a, b2base);
-            for (int n1 = 0; n1 < AC::PCN; ++n1) vi[static_cast<size_t>(w) * AC::PCN + n1] = psi[static_cast<size_t>(i) * m_points + x.gofs + AC::QC * n1];
-        }
+        std::fill(accj.begin(), accj.end(), 0.0);
+        std::fill(accl.begin(), accl.end(), 0.0);
+        stage_lines(j, res.data(), a, b2base);
+        stage_lines(lsafe, res.data() + AC::LINES * AC::LS, a, b2base);
         for (int t = 0; t < count; ++t) {
             for (int w = 0; w < AC::ITEMS_POS; ++w) {
                 const ColIdx x = col_index<AC, true>(w, a, b2base, na);
@@ -115,26 +114,26 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
                 c1_compute<AC>(SC.data() + x.seg, twc + x.k1 * AC::QC, x.k1);
             }
             const XformDesc d = desc[t];
-            stage_operands(d, a, b2base);
+            stage_lines(d.i, op.data(), a, b2base);
             double e1 = 0.0, e2 = 0.0;
             for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
                 const LineQIdx x = lineq_index<AC, true>(w, a, b2base);
-                c2_compute<AC>(SC.data() + x.row, d, fi, &vi[static_cast<size_t>(w) * AC::PCN], &op[x.op], &op[AC::LINES * AC::LS + x.op],
-                               &acc[static_cast<size_t>(w) * AC::PCN], e1, e2);
+                c2_compute<AC>(SC.data() + x.row, d, l, fj, fl, &res[x.op], &res[AC::LINES * AC::LS + x.op], &op[x.op],
+                               &accj[static_cast<size_t>(w) * AC::PCN], &accl[static_cast<size_t>(w) * AC::PCN], e1, e2);
             }
             e_out[2 * t] += e1;
             e_out[2 * t + 1] += e2;
-            for (int slot = 0; slot < 2; ++slot) {
-                const int orb = slot ? d.l : d.j;
-                if (orb < 0 || orb == i) continue;
-                for (int l = 0; l < AC::LINES; ++l)
+            if (d.flags != 0 && d.i != j && d.i != l)
+                for (int ln = 0; ln < AC::LINES; ++ln)
                     for (int c = 0; c < AC::NC; ++c)
-                        kpsi[static_cast<size_t>(orb) * m_points + line_offset<AC>(l, a, b2base) + c] += op[(slot * AC::LINES + l) * AC::LS + c];
-            }
+                        kpsi[static_cast<size_t>(d.i) * m_points + line_offset<AC>(ln, a, b2base) + c] += op[ln * AC::LS + c];
         }
         for (int w = 0; w < AC::ITEMS_LINE_Q; ++w) {
             const LineQIdx x = lineq_index<AC, true>(w, a, b2base);
-            for (int n1 = 0; n1 < AC::PCN; ++n1) kpsi[static_cast<size_t>(i) * m_points + x.gofs + AC::QC * n1] -= acc[static_cast<size_t>(w) * AC::PCN + n1];
+            for (int n1 = 0; n1 < AC::PCN; ++n1) {
+                kpsi[static_cast<size_t>(j) * m_points + x.gofs + AC::QC * n1] -= accj[static_cast<size_t>(w) * AC::PCN + n1];
+                if (l >= 0) kpsi[static_cast<size_t>(l) * m_points + x.gofs + AC::QC * n1] -= accl[static_cast<size_t>(w) * AC::PCN + n1];
+            }
         }
     }
     return 0;
@@ -142,14 +141,14 @@ static int emu_batch(const double* psi, double* kpsi, int i, double fi, int coun
 
 #define EMU_CASE(TA_, TB_, TC_, FREE_, G_, CH_)                                                              \
     if (ta == TA_ && tb == TB_ && tc == TC_ && free_bc == FREE_ && g == G_ && chunk == CH_)                    \
-        return emu_batch<TA_, TB_, TC_, FREE_ != 0, G_, CH_>(psi, kpsi, i, fi, count, desc, twa, twc, rootsb, ks, e_out);
+        return emu_batch<TA_, TB_, TC_, FREE_ != 0, G_, CH_>(psi, kpsi, j, l, fj, fl, count, desc, twa, twc, rootsb, ks, e_out);
 
 extern "C" int exx_emu_batch(int ta, int tb, int tc, int free_bc, int g, int chunk, const double* psi, double* kpsi,
-                             int i, double fi, int count, const int* jl /*[count][2]*/, const double* fjl /*[count][2]*/,
-                             const double* twa_, const double* twc_, const double* rootsb_, const double* ks,
-                             double* e_out) {
+                             int j, int l, double fj, double fl, int count, const int* iflags /*[count][2]*/,
+                             const double* fis /*[count]*/, const double* twa_, const double* twc_, const double* rootsb_,
+                             const double* ks, double* e_out) {
     std::vector<XformDesc> dv(count);
-    for (int t = 0; t < count; ++t) { dv[t].j = jl[2 * t]; dv[t].l = jl[2 * t + 1]; dv[t].fj = fjl[2 * t]; dv[t].fl = fjl[2 * t + 1]; }
+    for (int t = 0; t < count; ++t) { dv[t].i = iflags[2 * t]; dv[t].flags = iflags[2 * t + 1]; dv[t].fi = fis[t]; }
     const XformDesc* desc = dv.data();
     const double2* twa = reinterpret_cast<const double2*>(twa_);
     const double2* twc = reinterpret_cast<const double2*>(twc_);

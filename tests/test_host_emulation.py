@@ -41,7 +41,7 @@ def _build():
 def emu():
     lib = C.CDLL(_build())
     dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int)
-    lib.exx_emu_batch.argtypes = [C.c_int] * 6 + [dp, dp, C.c_int, C.c_double, C.c_int, ip, dp, dp, dp, dp, dp, dp]
+    lib.exx_emu_batch.argtypes = [C.c_int] * 6 + [dp, dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, ip, dp, dp, dp, dp, dp, dp]
     return lib
 
 
@@ -74,37 +74,40 @@ def test_emulated_batch_matches_oracle(emu, ta, tb, tc, free, G, chunk):
     psi = np.ascontiguousarray(w["psi"].numpy())
     o = Oracle(dims, w["spec"].spacing, "free" if free else "periodic", w["kernel"])
     occ = np.array([2.0, 1.5, 0.75, 1.0])[:n_orb]
-    i = 1
-    # the same-i batch of row i: pairs (1,1),(1,2) packed, then (1,3) alone (or just the first transform if N=3)
-    jl = [(1, 2), (3, -1)] if n_orb == 4 else [(1, 2)]
-    count = len(jl)
-    jl_arr = np.array(jl, dtype=np.int32)
-    fjl = np.array([[occ[j], occ[l] if l >= 0 else 0.0] for j, l in jl])
+    # the same-(j,l) batch of block-row {0,1}: i = 0 carries only the diagonal pair (0,0); i = 1 the pairs (0,1), (1,1);
+    # i >= 2 the pairs (0,i), (1,i).  N = 3 cases also run the odd tail block-row {2} (l = -1).
+    batches = [(0, 1, [(i, 1 if i == 0 else 3) for i in range(n_orb)])]
+    if n_orb == 3:
+        batches.append((2, -1, [(2, 1)]))
     khat = o.khat()
     T_tot = ta * tb * tc
     ks = np.ascontiguousarray(khat.real[: ta // 2 + 1, : tb // 2 + 1, : tc // 2 + 1]) / T_tot
     kpsi = np.zeros_like(psi)
-    e_out = np.zeros(2 * count)
     twa, twc, rootsb = _tw(ta), _tw(tc), _roots(tb)
     d = lambda x: x.ctypes.data_as(C.POINTER(C.c_double))
-    rc = emu.exx_emu_batch(ta, tb, tc, free, G, chunk, d(psi), d(kpsi), i, float(occ[i]), count,
-                           jl_arr.ctypes.data_as(C.POINTER(C.c_int)), d(fjl), d(twa.view(np.float64)),
-                           d(twc.view(np.float64)), d(rootsb.view(np.float64)), d(ks), d(e_out))
-    assert rc == 0, "case not instantiated in tests/emu/emu_passes.cu"
     ref = np.zeros_like(psi)
-    e_ref = []
-    for j, l in jl:
-        for slot in (j, l):
-            if slot < 0:
-                e_ref.append(0.0)
-                continue
-            rho = psi[i] * psi[slot]
-            v = o.poisson(rho)
-            ref[i] -= occ[slot] * v * psi[slot]
-            if slot != i:
-                ref[slot] -= occ[i] * v * psi[i]
-            e_ref.append(np.sum(rho * v))
+    for j, l, xf in batches:
+        count = len(xf)
+        iflags = np.array(xf, dtype=np.int32)
+        fis = np.array([occ[i] for i, _ in xf])
+        e_out = np.zeros(2 * count)
+        rc = emu.exx_emu_batch(ta, tb, tc, free, G, chunk, d(psi), d(kpsi), j, l, float(occ[j]), float(occ[l]) if l >= 0 else 0.0,
+                               count, iflags.ctypes.data_as(C.POINTER(C.c_int)), d(fis), d(twa.view(np.float64)),
+                               d(twc.view(np.float64)), d(rootsb.view(np.float64)), d(ks), d(e_out))
+        assert rc == 0, "case not instantiated in tests/emu/emu_passes.cu"
+        e_ref = []
+        for i, flags in xf:
+            for bit, x in ((1, j), (2, l)):
+                if not flags & bit:
+                    e_ref.append(0.0)
+                    continue
+                rho = psi[x] * psi[i]
+                v = o.poisson(rho)
+                ref[x] -= occ[i] * v * psi[i]
+                if x != i:
+                    ref[i] -= occ[x] * v * psi[x]
+                e_ref.append(np.sum(rho * v))
+        e_ref = np.array(e_ref)
+        assert np.max(np.abs(e_out - e_ref)) <= 1e-12 * np.max(np.abs(e_ref))
     scale = np.max(np.abs(ref))
     assert np.max(np.abs(kpsi - ref)) <= 1e-12 * scale
-    e_ref = np.array(e_ref)
-    assert np.max(np.abs(e_out - e_ref)) <= 1e-12 * np.max(np.abs(e_ref))
