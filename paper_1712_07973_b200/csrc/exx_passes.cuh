@@ -522,16 +522,17 @@ EXX_HD void b1_compute(double2* colp, const double2* tw, int tws) {
 template <class C>
 EXX_HD void b2_compute(double2* colp, const double* kcol, const double2* tw, int tws, int k1) {
     double xr[C::QA], xi[C::QA];
+    double kv[C::QA];                                          // issued first: the L2 latency hides behind the forward DFT
+#pragma unroll
+    for (int k2 = 0; k2 < C::QA; ++k2) {
+        const int ka = k1 + C::PA * k2;
+        kv[k2] = ld_ro(kcol + (ka <= C::TA - ka ? ka : C::TA - ka));
+    }
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = colp[n2 * C::RS]; xr[n2] = v.x; xi[n2] = v.y; }
     Dft<C::QA>::run(xr, xi);
 #pragma unroll
-    for (int k2 = 0; k2 < C::QA; ++k2) {
-        const int ka = k1 + C::PA * k2;
-        const int sa = ka <= C::TA - ka ? ka : C::TA - ka;
-        const double kv = ld_ro(kcol + sa);
-        xr[k2] *= kv; xi[k2] *= kv;
-    }
+    for (int k2 = 0; k2 < C::QA; ++k2) { xr[k2] *= kv[k2]; xi[k2] *= kv[k2]; }
     dft_inv<C::QA, false>(xr, xi);
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) {
