@@ -100,6 +100,17 @@ exx_status exx_get_pair_energies(exx_plan *plan, double *e_host);
  */
 exx_status exx_schedule_pairs(int n_orb, const double *occ_host, long long *n_pairs, long long *n_transforms);
 
+/*
+ * exx_schedule_list -- HOST-only listing of the same schedule, cut into batches of at most max_batch transforms
+ * (max_batch < 1: unlimited).  Row t of xforms_host [capacity][5] receives {j, l, i, flags, batch}: the transform
+ * carries the pairs (j,i) in its real part (flags bit 0) and (l,i) in its imaginary part (flags bit 1) of the
+ * co-density z = psi_i psi_j + i psi_i psi_l (Eq. 8); j, l are the two resident orbitals of batch
+ * `batch` (l = -1: none).  *n_transforms receives the total; at most `capacity` rows are written (xforms_host may
+ * be NULL when capacity is 0).  Every unordered pair that is not doubly empty appears exactly once.
+ */
+exx_status exx_schedule_list(int n_orb, const double *occ_host, int max_batch, int *xforms_host, long long capacity,
+                             long long *n_transforms);
+
 /* Transform-grid lengths (n or 2n) of a plan and the bytes of device workspace it owns. */
 exx_status exx_plan_transform_dims(const exx_plan *plan, int tdims[3]);
 size_t     exx_plan_workspace_bytes(const exx_plan *plan);

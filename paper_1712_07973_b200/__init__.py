@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     exx_apply,
     exx_plan_create,
     exx_plan_destroy,
+    exx_schedule_list,
     exx_schedule_pairs,
     exx_version,
     library_path,

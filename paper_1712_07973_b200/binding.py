@@ -22,7 +22,7 @@ _STATUS = ["EXX_OK", "EXX_ERR_INVALID_ARG", "EXX_ERR_UNSUPPORTED_SIZE", "EXX_ERR
 
 EXPORTS = [
     "exx_plan_create", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_get_pair_energies",
-    "exx_schedule_pairs", "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count",
+    "exx_schedule_pairs", "exx_schedule_list", "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count",
     "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version",
 ]
 
@@ -60,6 +60,8 @@ def load_library():
     lib.exx_get_pair_energies.restype = C.c_int
     lib.exx_schedule_pairs.argtypes = [C.c_int, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     lib.exx_schedule_pairs.restype = C.c_int
+    lib.exx_schedule_list.argtypes = [C.c_int, _dp, C.c_int, _ip, C.c_longlong, C.POINTER(C.c_longlong)]
+    lib.exx_schedule_list.restype = C.c_int
     lib.exx_plan_transform_dims.argtypes = [C.c_void_p, _ip]
     lib.exx_plan_transform_dims.restype = C.c_int
     lib.exx_plan_workspace_bytes.argtypes = [C.c_void_p]
@@ -96,6 +98,22 @@ def exx_schedule_pairs(occ: Sequence[float]):
     if st:
         raise ExxError(st, "exx_schedule_pairs")
     return n_pairs.value, n_x.value
+
+
+def exx_schedule_list(occ: Sequence[float], max_batch: int = 0):
+    """int32 array [n_transforms][5] of {j, l, i, flags, batch} -- host only, no GPU needed (see include/exx.h)."""
+    occ = np.ascontiguousarray(np.asarray(occ, dtype=np.float64))
+    lib = load_library()
+    n_x = C.c_longlong()
+    st = lib.exx_schedule_list(int(occ.size), occ.ctypes.data_as(_dp), int(max_batch), None, 0, C.byref(n_x))
+    if st:
+        raise ExxError(st, "exx_schedule_list")
+    out = np.zeros((n_x.value, 5), dtype=np.int32)
+    if n_x.value:
+        st = lib.exx_schedule_list(int(occ.size), occ.ctypes.data_as(_dp), int(max_batch), out.ctypes.data_as(_ip), n_x.value, C.byref(n_x))
+        if st:
+            raise ExxError(st, "exx_schedule_list")
+    return out
 
 
 class ExxPlan:

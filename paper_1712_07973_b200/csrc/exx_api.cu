@@ -451,6 +451,25 @@ exx_status exx_schedule_pairs(int n_orb, const double* occ_host, long long* n_pa
     return EXX_OK;
 }
 
+exx_status exx_schedule_list(int n_orb, const double* occ_host, int max_batch, int* xforms_host, long long capacity,
+                             long long* n_transforms) {
+    if (n_orb < 1 || !occ_host || !n_transforms || capacity < 0 || (capacity > 0 && !xforms_host)) return EXX_ERR_INVALID_ARG;
+    try {
+        Schedule s = build_schedule(n_orb, occ_host, max_batch < 1 ? 1 << 30 : max_batch);
+        *n_transforms = static_cast<long long>(s.xforms.size());
+        for (size_t b = 0; b < s.batches.size(); ++b) {
+            const Batch& bt = s.batches[b];
+            for (int t = bt.first; t < bt.first + bt.count && t < capacity; ++t) {
+                int* row = xforms_host + static_cast<size_t>(t) * 5;
+                row[0] = bt.j; row[1] = bt.l; row[2] = s.xforms[t].i; row[3] = s.xforms[t].flags; row[4] = static_cast<int>(b);
+            }
+        }
+    } catch (const std::bad_alloc&) {
+        return EXX_ERR_ALLOC;
+    }
+    return EXX_OK;
+}
+
 exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spacing[3], exx_bc bc, const double* kernel_host,
                            int max_orbitals, void* cuda_stream) {
     g_create_error.clear();

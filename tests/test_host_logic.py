@@ -33,8 +33,8 @@ def test_p10_pair_counts_match_table1():
         n_orb, solves = int(n_orb), int(solves)
         n_pairs, n_x = exx.exx_schedule_pairs([2.0] * n_orb)
         assert n_pairs == solves == n_orb * (n_orb + 1) // 2
-        # rows with an odd number of pairs end with a half-empty transform
-        assert n_x == sum((n_orb - i + 1) // 2 for i in range(n_orb))
+        # block-row {j, j+1} holds one transform per streamed orbital i >= j (i = j carries only the diagonal pair)
+        assert n_x == sum(n_orb - j for j in range(0, n_orb, 2))
 
 
 def test_scheduler_skips_only_doubly_empty_pairs():
@@ -44,6 +44,34 @@ def test_scheduler_skips_only_doubly_empty_pairs():
     assert n_pairs == expect == 9
     assert exx.exx_schedule_pairs([0.0, 0.0]) == (0, 0)
     assert exx.exx_schedule_pairs([1.0]) == (1, 1)
+
+
+@pytest.mark.parametrize("occ,max_batch", [([2.0] * 7, 0), ([2.0] * 8, 3), ([2.0, 0.0, 1.0, 0.0, 0.0, 1.5], 2), ([0.0, 0.0, 1.0], 0),
+                                           ([1.0], 0), ([2.0] * 33, 5)])
+def test_schedule_covers_every_pair_exactly_once(occ, max_batch):
+    """Row-pair schedule (include/exx.h exx_schedule_list): every unordered pair that is not doubly empty is carried by
+    exactly one transform slot; batches share (j,l), never stream j or l as an update target twice, and respect max_batch."""
+    n = len(occ)
+    rows = exx.exx_schedule_list(occ, max_batch)
+    seen = {}
+    per_batch = {}
+    for j, l, i, flags, b in rows.tolist():
+        assert flags in (1, 2, 3) and 0 <= j <= i < n and (l == -1 or l == j + 1)
+        per_batch.setdefault(b, []).append((j, l, i))
+        if flags & 1:
+            seen[(j, i)] = seen.get((j, i), 0) + 1
+        if flags & 2:
+            assert l >= 0 and i >= l
+            seen[(l, i)] = seen.get((l, i), 0) + 1
+    expect = {(x, y) for x in range(n) for y in range(x, n) if not (occ[x] == 0 and occ[y] == 0)}
+    assert set(seen) == expect and all(v == 1 for v in seen.values())
+    assert exx.exx_schedule_pairs(occ) == (len(expect), len(rows))
+    for b, items in per_batch.items():
+        assert len({(j, l) for j, l, _ in items}) == 1, "a batch shares its resident orbitals"
+        streamed = [i for _, _, i in items]
+        assert len(set(streamed)) == len(streamed), "K psi_i targets of a batch are distinct"
+        if max_batch > 0:
+            assert len(items) <= max_batch
 
 
 def test_status_codes_without_compute():
