@@ -38,7 +38,7 @@ cudaError_t query_pass_c(const Geometry& g, KernelInfo* info);
 
 // Compile-time tuning shared by the instantiation files -------------------------------------------------------
 constexpr int kSmemPerSM = 227 * 1024;                     // usable shared memory per SM (and per CTA, opt-in)
-constexpr int kMaxSmemAC = 220 * 1024;                     // passes A / C: work buffer(s) + operand stages
+constexpr int kMaxSmemAC = 216 * 1024;                     // passes A / C: work buffer(s) + operand stages
 constexpr int round_up32(int x) { return (x + 31) / 32 * 32; }
 constexpr int imin(int a, int b) { return a < b ? a : b; }
 constexpr int imax(int a, int b) { return a > b ? a : b; }
@@ -70,8 +70,8 @@ constexpr int pick_g(bool pass_c, int max_bytes) {
 // resident CTAs per SM to compile for: limited by shared memory, by a register floor per thread, and by `cap`; among
 // the admissible counts the one that wastes the fewest CTA slots in the last wave of a cubic grid's `tiles` CTAs on 148
 // SMs wins (a tile is a long loop over the batch, so a ragged last wave costs a whole loop), ties -> more CTAs
-constexpr int pick_minb(int smem, int nt, int reg_floor, int cap, int tiles) {
-    const int maxb = imax(1, imin(imin(kSmemPerSM / (smem + 1024), 65536 / (nt * reg_floor)), cap));
+constexpr int pick_minb(int smem, int nt, int reg_floor, int cap, int tiles) {       // smem: dynamic + static bytes
+    const int maxb = imax(1, imin(imin((kSmemPerSM + 1024) / (smem + 1024), 65536 / (nt * reg_floor)), cap));
     int best = 1, best_eff = -1;
     for (int b = 1; b <= maxb; ++b) {
         const int slots = 148 * b, waves = (tiles + slots - 1) / slots;
@@ -92,14 +92,14 @@ struct TuneAC {
     static constexpr int NBUF_C = smem_ac_bytes<TC, TB, FREE>(G_C, 1, true, 2) <= kMaxSmemAC ? 2 : 1;
     static constexpr int NSTG_C = smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, NBUF_C) <= kMaxSmemAC ? 2 : 1;
     static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true, NBUF_C);
-    static constexpr int MINB_C = pick_minb(SMEM_C, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
+    static constexpr int MINB_C = pick_minb(SMEM_C + (TC + TB) * 16 + 256, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A
     static constexpr int G_A = pick_g<TC, TB, FREE>(false, kMaxSmemAC / 3);
     using CfgA = CfgAC<TC, TB, FREE, G_A, CHUNK>;
     static constexpr int NT_A = imax(32, round_up32(imax(CfgA::ITEMS_LINE_Q, imin(CfgA::ITEMS_POS, 256))));
     static constexpr int NSTG_A = 2;
     static constexpr int SMEM_A = smem_ac_bytes<TC, TB, FREE>(G_A, NSTG_A, false);
-    static constexpr int MINB_A = pick_minb(SMEM_A, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
+    static constexpr int MINB_A = pick_minb(SMEM_A + (TC + TB) * 16 + 64, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
     static_assert(SMEM_C <= kMaxSmemAC && SMEM_A <= kMaxSmemAC, "tile does not fit shared memory");
 };
 

@@ -230,7 +230,7 @@ EXX_HD void a0_compute(const double* vj, const double* vl, const double* pi, int
     dft_fwd<C::PC, C::FREE>(xr, xi);
 #pragma unroll
     for (int k1 = 0; k1 < C::PC; ++k1) {
-        if (k1 > 0) cmul(xr[k1], xi[k1], ld_ro(tw + k1 * C::QC));
+        if (k1 > 0) cmul(xr[k1], xi[k1], tw[k1 * C::QC]);
         row[k1 * C::QCP] = make_double2(xr[k1], xi[k1]);
     }
 }
@@ -258,7 +258,7 @@ EXX_HD void a2_compute(const double2* col, const double2* tw, double2* dst, size
     dft_fwd<C::R1, C::FREE>(xr, xi);
 #pragma unroll
     for (int q = 0; q < C::R1; ++q) {
-        if (q > 0) cmul(xr[q], xi[q], ld_ro(tw + q));
+        if (q > 0) cmul(xr[q], xi[q], tw[q]);
         dst[q * qstride] = make_double2(xr[q], xi[q]);
     }
 }
@@ -272,23 +272,23 @@ EXX_HD void c0_compute(double2* col, const double2* tw) {
     for (int q = 0; q < C::R1; ++q) {
         double2 v = col[q * C::ROW];
         xr[q] = v.x; xi[q] = v.y;
-        if (q > 0) cmul_conj(xr[q], xi[q], ld_ro(tw + q));
+        if (q > 0) cmul_conj(xr[q], xi[q], tw[q]);
     }
     dft_inv<C::R1, C::FREE>(xr, xi);
 #pragma unroll
     for (int b1 = 0; b1 < C::NB1; ++b1) col[b1 * C::ROW] = make_double2(xr[b1], xi[b1]);
 }
 
-// ---- C1: inverse stage over k2 (Q-point) of the c axis + conj twiddle.  tw = twc + k1*QC
+// ---- C1: inverse stage over k2 (Q-point) of the c axis + conj twiddle W_TC^{-n2 k1} = conj(tw[n2*tws])
 template <class C>
-EXX_HD void c1_compute(double2* seg, const double2* tw, int k1) {
+EXX_HD void c1_compute(double2* seg, const double2* tw, int tws, int k1) {
     double xr[C::QC], xi[C::QC];
 #pragma unroll
     for (int k2 = 0; k2 < C::QC; ++k2) { double2 v = seg[k2]; xr[k2] = v.x; xi[k2] = v.y; }
     dft_inv<C::QC, false>(xr, xi);
 #pragma unroll
     for (int n2 = 0; n2 < C::QC; ++n2) {
-        if (k1 > 0) cmul_conj(xr[n2], xi[n2], ld_ro(tw + n2));
+        if (k1 > 0) cmul_conj(xr[n2], xi[n2], tw[n2 * tws]);
         seg[n2] = make_double2(xr[n2], xi[n2]);
     }
 }
@@ -592,6 +592,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     double2* const S = reinterpret_cast<double2*>(smem_raw);
     double* const OP = reinterpret_cast<double*>(S + C::SMEM_A);
     __shared__ uint64_t full[NSTG];
+    __shared__ double2 s_twc[C::TC], s_twb[C::TB];         // twiddle tables (shared-memory reads instead of L1 hits)
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
     constexpr int NI0 = ceil_div(C::ITEMS_LINE_Q, NT), NI1 = ceil_div(C::ITEMS_LINE_P, NT), NI2 = ceil_div(C::ITEMS_POS, NT);
@@ -600,6 +601,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
         for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
+    for (int x = tid; x < C::TC; x += NT) s_twc[x] = g.twc[x];
+    for (int x = tid; x < C::TB; x += NT) s_twb[x] = g.twb[x];
     __syncthreads();
     if (tid < 32)
         for (int t = 0; t < NSTG && t < g.count; ++t)
@@ -633,7 +636,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
             if (tid + m * NT < C::ITEMS_LINE_Q)
-                a0_compute<C>(vj[m], vl[m], stage + q0[m].op, flags, S + q0[m].row, g.twc + q0[m].n2);
+                a0_compute<C>(vj[m], vl[m], stage + q0[m].op, flags, S + q0[m].row, s_twc + q0[m].n2);
         __syncthreads();
         if (tid < 32 && t + NSTG < g.count)                    // the stage has been consumed: refill it
             issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
@@ -644,7 +647,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
         double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
 #pragma unroll
         for (int m = 0; m < NI2; ++m)
-            if (tid + m * NT < C::ITEMS_POS) a2_compute<C>(S + c2[m].col, g.twb + c2[m].b2 * C::R1, w1t + c2[m].w1, qstride);
+            if (tid + m * NT < C::ITEMS_POS) a2_compute<C>(S + c2[m].col, s_twb + c2[m].b2 * C::R1, w1t + c2[m].w1, qstride);
         __syncthreads();
     }
 }
@@ -751,6 +754,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     __shared__ uint64_t full[NSTG];
     __shared__ uint64_t resbar;
     __shared__ double red[2][NT / 32];
+    __shared__ double2 s_twct[C::TC], s_twb[C::TB];        // twiddle tables; the c-axis one transposed to [n2*PC + k1]
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
     constexpr int NI0 = ceil_div(C::ITEMS_POS, NT), NI1 = ceil_div(C::ITEMS_LINE_P, NT), NI2 = ceil_div(C::ITEMS_LINE_Q, NT);
@@ -760,6 +764,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         mbar_init(&resbar, 1);
         mbar_fence_init();
     }
+    for (int x = tid; x < C::TC; x += NT) s_twct[(x % C::QC) * C::PC + x / C::QC] = g.twc[x];
+    for (int x = tid; x < C::TB; x += NT) s_twb[x] = g.twb[x];
     __syncthreads();
 
     ColIdx c0[NI0];
@@ -818,11 +824,11 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         }
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
-            if (tid + m * NT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, g.twb + c0[m].b2 * C::R1);
+            if (tid + m * NT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, s_twb + c0[m].b2 * C::R1);
         __syncthreads();
 #pragma unroll
         for (int m = 0; m < NI1; ++m)
-            if (tid + m * NT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, g.twc + p1[m].k1 * C::QC, p1[m].k1);
+            if (tid + m * NT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, s_twct + p1[m].k1, C::PC, p1[m].k1);
         __syncthreads();
         if (t == 0) mbar_wait(&resbar, 0);                 // psi_j / psi_l lines of the tile
         mbar_wait(&full[s], (t / NSTG) & 1);               // psi_i lines of transform t have landed

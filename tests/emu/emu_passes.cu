@@ -111,7 +111,7 @@ static int emu_batch(const double* psi, double* kpsi, int j, int l, double fj, d
             }
             for (int w = 0; w < AC::ITEMS_LINE_P; ++w) {
                 const LinePIdx x = linep_index<AC, true>(w);
-                c1_compute<AC>(SC.data() + x.seg, twc + x.k1 * AC::QC, x.k1);
+                c1_compute<AC>(SC.data() + x.seg, twc + x.k1 * AC::QC, 1, x.k1);
             }
             const XformDesc d = desc[t];
             stage_lines(d.i, op.data(), a, b2base);
