@@ -89,7 +89,12 @@ struct TuneAC {
     using CfgC = CfgAC<TC, TB, FREE, G_C, CHUNK>;
     static constexpr int NT_C = imax(32, round_up32(imax(CfgC::ITEMS_LINE_Q, imin(CfgC::ITEMS_POS, 256))));
     // double-buffered W1 tile where it fits next to one operand stage and the resident lines, else single-buffered
-    static constexpr int NBUF_C = smem_ac_bytes<TC, TB, FREE>(G_C, 1, true, 2) <= kMaxSmemAC ? 2 : 1;
+    // single-buffered W1 tile if that is what lets two CTAs share an SM (the other CTA then covers the gather), else
+    // double-buffered where it fits next to one operand stage and the resident lines
+    static constexpr int kStaticC = (TC + TB) * 16 + 1280;
+    static constexpr int NBUF_C = (smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, 2) + kStaticC) * 2 > kSmemPerSM + 1024 &&
+                                  (smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, 1) + kStaticC) * 2 <= kSmemPerSM + 1024 ? 1 :
+                                  (smem_ac_bytes<TC, TB, FREE>(G_C, 1, true, 2) <= kMaxSmemAC ? 2 : 1);
     static constexpr int NSTG_C = smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, NBUF_C) <= kMaxSmemAC ? 2 : 1;
     static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true, NBUF_C);
     static constexpr int MINB_C = pick_minb(SMEM_C + (TC + TB) * 16 + 256, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
