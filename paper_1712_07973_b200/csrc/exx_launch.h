@@ -75,7 +75,7 @@ constexpr int pick_minb(int smem, int nt, int reg_floor, int cap, int tiles) {  
     int best = 1, best_eff = -1;
     for (int b = 1; b <= maxb; ++b) {
         const int slots = 148 * b, waves = (tiles + slots - 1) / slots;
-        const int eff = tiles * 1000 / (waves * slots) + (b > 1 ? 30 : 0);     // co-residency itself is worth a little
+        const int eff = tiles * 1000 / (waves * slots) + (b > 1 ? 100 : 0);    // co-residency itself is worth 10 %
         if (eff >= best_eff) { best_eff = eff; best = b; }
     }
     return best;
@@ -89,13 +89,15 @@ struct TuneAC {
     using CfgC = CfgAC<TC, TB, FREE, G_C, CHUNK>;
     static constexpr int NT_C = imax(32, round_up32(imax(CfgC::ITEMS_LINE_Q, imin(CfgC::ITEMS_POS, 256))));
     // double-buffered W1 tile where it fits next to one operand stage and the resident lines, else single-buffered
-    // single-buffered W1 tile if that is what lets two CTAs share an SM (the other CTA then covers the gather), else
-    // double-buffered where it fits next to one operand stage and the resident lines
+    // W1 tile buffers (NBUF) and operand stages (NSTG): the deepest pipeline with which two CTAs share an SM (the other
+    // CTA then covers what a shallower pipeline exposes), else the deepest one that fits at all
     static constexpr int kStaticC = (TC + TB) * 16 + 1280;
-    static constexpr int NBUF_C = (smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, 2) + kStaticC) * 2 > kSmemPerSM + 1024 &&
-                                  (smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, 1) + kStaticC) * 2 <= kSmemPerSM + 1024 ? 1 :
-                                  (smem_ac_bytes<TC, TB, FREE>(G_C, 1, true, 2) <= kMaxSmemAC ? 2 : 1);
-    static constexpr int NSTG_C = smem_ac_bytes<TC, TB, FREE>(G_C, 2, true, NBUF_C) <= kMaxSmemAC ? 2 : 1;
+    static constexpr bool two_fit(int nbuf, int nstg) {
+        return (smem_ac_bytes<TC, TB, FREE>(G_C, nstg, true, nbuf) + kStaticC) * 2 <= kSmemPerSM + 1024;
+    }
+    static constexpr bool one_fits(int nbuf, int nstg) { return smem_ac_bytes<TC, TB, FREE>(G_C, nstg, true, nbuf) <= kMaxSmemAC; }
+    static constexpr int NBUF_C = two_fit(2, 2) ? 2 : two_fit(1, 2) ? 1 : two_fit(1, 1) ? 1 : (one_fits(2, 2) || one_fits(2, 1)) ? 2 : 1;
+    static constexpr int NSTG_C = two_fit(2, 2) ? 2 : two_fit(1, 2) ? 2 : two_fit(1, 1) ? 1 : one_fits(NBUF_C, 2) ? 2 : 1;
     static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true, NBUF_C);
     static constexpr int MINB_C = pick_minb(SMEM_C + (TC + TB) * 16 + 256, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A

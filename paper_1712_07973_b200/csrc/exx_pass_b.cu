@@ -74,6 +74,15 @@ cudaError_t query_pass_b(const Geometry& g, KernelInfo* info) {
     return dispatch_b(g, args, 0, nullptr, info, false);
 }
 
+#ifdef EXX_DEBUG_TIMING
+extern "C" void exx_debug_b_read(long long* out16) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out16, g_dbg_b, sizeof(long long) * 16);
+    long long z[16] = {0};
+    cudaMemcpyToSymbol(g_dbg_b, z, sizeof(z));
+}
+#endif
+
 bool length_supported(int t) {
     return t == 16 || t == 32 || t == 64 || t == 96 || t == 128 || t == 192 || t == 256;
 }

@@ -55,11 +55,11 @@ template <> struct BSplit<32>  { static constexpr int R1 = 8,  R2 = 4;  };
 template <> struct BSplit<64>  { static constexpr int R1 = 8,  R2 = 8;  };
 template <> struct BSplit<96>  { static constexpr int R1 = 8,  R2 = 12; };
 template <> struct BSplit<128> { static constexpr int R1 = 16, R2 = 8;  };
-template <> struct BSplit<192> { static constexpr int R1 = 16, R2 = 12; };
+template <> struct BSplit<192> { static constexpr int R1 = 12, R2 = 16; };   // 12 lines per A/C tile: two CTAs per SM
 template <> struct BSplit<256> { static constexpr int R1 = 16, R2 = 16; };
 
 constexpr int r2_of(int tb) {
-    return tb == 16 ? 4 : tb == 32 ? 4 : tb == 64 ? 8 : tb == 96 ? 12 : tb == 128 ? 8 : tb == 192 ? 12 : 16;
+    return tb == 16 ? 4 : tb == 32 ? 4 : tb == 64 ? 8 : tb == 96 ? 12 : tb == 128 ? 8 : tb == 192 ? BSplit<192>::R2 : 16;
 }
 constexpr int split_p(int t) { return t == 16 ? 4 : t == 32 ? 4 : t == 64 ? 8 : t == 96 ? 8 : t == 128 ? 8 : t == 192 ? 12 : 16; }
 constexpr int split_q(int t) { return t / split_p(t); }
@@ -652,6 +652,13 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     }
 }
 
+#ifdef EXX_DEBUG_TIMING
+static __device__ long long g_dbg_b[16];
+#define EXX_DBG(k) do { if (dbg_on) { const long long now = clock64(); dbg_acc[k] += now - dbg_prev; dbg_prev = now; } } while (0)
+#else
+#define EXX_DBG(k) do { } while (0)
+#endif
+
 // Pass B.  Persistent CTAs over the (pch, q, t) blocks of the launch, t fastest (CTAs that run at the same time
 // share a K^ slice in L2).  The next block lands in a separate buffer by TMA bulk row copies while the current one is
 // transformed.  B0 / B4 map a thread to the rows (a, pin) it alone reads and writes, and the a-axis phases B1..B3 map
@@ -690,19 +697,28 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
     };
     if (tid < 32 && static_cast<int>(blockIdx.x) < g.ntiles) issue_block_load(blockIdx.x);
 
+#ifdef EXX_DEBUG_TIMING
+    const bool dbg_on = tid == 0 || tid == NT - 32;
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long dbg_prev = clock64();
+#endif
     int it = 0;
     for (int id = blockIdx.x; id < g.ntiles; id += gridDim.x, ++it) {
         const int rest = id / g.count;
         const int q = rest % C::R1, pch = rest / C::R1;
         double2* blk = block_ptr(id);
+        EXX_DBG(6);
         mbar_wait(&full, it & 1);
+        EXX_DBG(0);
 #pragma unroll
         for (int m = 0; m < NIO; ++m)
             if (tid + m * NT < C::ITEMS_IO) {
                 const IoIdx x = io_index<C>(tid + m * NT);
                 b0_compute<C>(L + x.l, W + x.s);
             }
+        EXX_DBG(1);
         __syncthreads();
+        EXX_DBG(2);
         if (tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
         for (int cg = wid; cg < C::NGRP; cg += NW) {
 #pragma unroll
@@ -726,14 +742,21 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
             for (int m = 0; m < NQ; ++m)
                 if (lane + m * 32 < C::ITEMS_Q) b3_compute<C>(W + colq_index<C>(cg, lane + m * 32).base);
         }
+        EXX_DBG(3);
         __syncthreads();
+        EXX_DBG(4);
 #pragma unroll
         for (int m = 0; m < NIO; ++m)
             if (tid + m * NT < C::ITEMS_IO) {
                 const IoIdx x = io_index<C>(tid + m * NT);
                 b4_compute<C>(W + x.s, blk + x.g);
             }
+        EXX_DBG(5);
     }
+#ifdef EXX_DEBUG_TIMING
+    if (dbg_on)
+        for (int k = 0; k < 8; ++k) atomicAdd(reinterpret_cast<unsigned long long*>(&g_dbg_b[(tid == 0 ? 0 : 8) + k]), static_cast<unsigned long long>(dbg_acc[k]));
+#endif
 }
 
 // Pass C.  One CTA per (a, b2-group) tile; it loops over the transforms of the same-(j,l) batch, keeps the K psi_j and
