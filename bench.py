@@ -38,16 +38,29 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def _ncu_traffic(config: str, pass_name: str):
-    """dram__bytes_read+write per launch of the dominant kernel from the committed ncu capture, or None."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+def _ncu_traffic(config: str, pass_name: str, xforms_per_launch: float):
+    """dram__bytes_read+write per launch of the dominant kernel from the committed `ncu --set full` capture
+    (profiles/r01_traffic.csv: config,pass,transforms_in_launch,dram_bytes), scaled to this run's mean launch size."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
     if not os.path.exists(path):
         return None
     try:
         with open(path) as fh:
-            return json.load(fh).get(config, {}).get(pass_name)
+            for line in fh:
+                f = line.strip().split(",")
+                if len(f) == 4 and f[0] == config and f[1] == pass_name:
+                    return float(f[3]) / float(f[2]) * xforms_per_launch
     except Exception:
         return None
+    return None
+
+
+def aggregate_over_ranks(step_ms_local: float, pairs_per_rank: int, world: int, all_reduce_max=None):
+    """Replicas-only scaling: every rank applies the whole operator to its own copy; the job's
+    time is the MAX over ranks (all_reduce_max: callable float -> float, identity for one rank) and the job's
+    throughput is the pairs of all ranks over that time."""
+    step_ms = all_reduce_max(step_ms_local) if (all_reduce_max is not None and world > 1) else step_ms_local
+    return step_ms, pairs_per_rank * world / (step_ms * 1e-3)
 
 
 class ClockSampler(threading.Thread):
@@ -244,11 +257,12 @@ def main():
     clocks = sampler.stop()
     plan.set_profiling(False)
     ex_value = float(ex_dev[0])
-    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
-    if distributed:
+    def all_reduce_max(x: float) -> float:
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    step_ms = float(t[0]) / args.steps
-    value = n_pairs * world / (step_ms * 1e-3)
+        return float(t[0])
+
+    step_ms, value = aggregate_over_ranks(elapsed_ms / args.steps, n_pairs, world, all_reduce_max if distributed else None)
 
     # ---- roofline of the dominant kernel (per-launch algorithmic bytes / mean launch duration)
     peak, peak_src = _peaks()
@@ -260,7 +274,8 @@ def main():
     dom_bytes_per_launch = per_x[dom_name] * n_xforms / max(1, pass_n[dom])
     achieved = dom_bytes_per_launch / (dom_ms_per_launch * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": f"pass_{dom_name.lower()}_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": _ncu_traffic(args.config, dom_name), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": _ncu_traffic(args.config, dom_name, n_xforms / max(1, pass_n[dom])),
+                "peak_source": peak_src,
                 "alg_bytes_per_launch": dom_bytes_per_launch, "ms_per_launch": dom_ms_per_launch,
                 "pass_ms_per_step": {k: float(v) for k, v in zip(["A", "B", "C", "reduce"], pass_ms)},
                 "pass_GBps": {k: float(per_x[k] * n_xforms / (pass_ms[i] * 1e-3) / 1e9) for i, k in enumerate(names)}}
