@@ -81,8 +81,9 @@ exx_status exx_apply_async(exx_plan *plan, int n_orb, const double *psi_dev, con
 
 /*
  * exx_apply_host -- end-to-end convenience: psi_host / kpsi_host are HOST buffers (pinned or pageable); the
- * library stages them through device memory it owns (host->device copy of psi, device->host copy of K psi),
- * on the plan's stream, and synchronises.  Same arithmetic as exx_apply.
+ * library stages them through device memory it owns (host->device copy of psi on the plan's stream; each K psi
+ * row is copied device->host on an internal copy stream as soon as its block-row has finished, overlapping the
+ * remaining pair solves when kpsi_host is pinned), and synchronises.  Same arithmetic as exx_apply.
  */
 exx_status exx_apply_host(exx_plan *plan, int n_orb, const double *psi_host, const double *occ_host,
                           double *kpsi_host, double *ex_host);

@@ -172,6 +172,8 @@ struct exx_plan {
     double* ex_dev;
     double* ex_pinned;
     cudaEvent_t upload_done;
+    cudaStream_t copy_stream;   // exx_apply_host: finished K psi rows leave while later block-rows compute
+    cudaEvent_t row_done, copy_done;
     double* psi_stage;
     double* kpsi_stage;
     size_t stage_elems;
@@ -353,7 +355,9 @@ exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
     return EXX_OK;
 }
 
-exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* occ_host, double* kpsi) {
+// kpsi_host != nullptr (exx_apply_host): K psi_j and K psi_l are final once the last batch of block-row {j,l} has run
+// (later block-rows only stream orbitals i > l), so their device-to-host copies overlap the remaining block-rows.
+exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* occ_host, double* kpsi, double* kpsi_host = nullptr) {
     // wait until the previous apply's descriptor upload has left the pinned staging buffers
     EXX_CUDA(p, cudaEventSynchronize(p->upload_done));
     Schedule sched = build_schedule(n_orb, occ_host, p->max_batch);
@@ -388,6 +392,7 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
         if (!p->profiling) return cudaSuccess;
         return cudaEventRecord(p->events[p->events_used++], s);
     };
+    std::vector<char> copied(kpsi_host ? n_orb : 0, 0);
     for (const Batch& b : sched.batches) {
         ac.desc = p->desc_dev + b.first;
         ac.j = b.j; ac.l = b.l; ac.fj = b.fj; ac.fl = b.fl; ac.count = b.count;
@@ -402,6 +407,24 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
         EXX_CUDA(p, cudaGetLastError());
         EXX_CUDA(p, mark());
         p->launches += 4;
+        const bool row_ends = (&b == &sched.batches.back()) || ((&b)[1].j != b.j);
+        if (kpsi_host && row_ends) {
+            const size_t rows = b.l >= 0 ? 2 : 1, off = static_cast<size_t>(b.j) * p->M;
+            EXX_CUDA(p, cudaEventRecord(p->row_done, s));
+            EXX_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->row_done, 0));
+            EXX_CUDA(p, cudaMemcpyAsync(kpsi_host + off, kpsi + off, rows * p->M * sizeof(double), cudaMemcpyDeviceToHost, p->copy_stream));
+            for (size_t r = 0; r < rows; ++r) copied[b.j + r] = 1;
+        }
+    }
+    if (kpsi_host) {                                       // rows of block-rows without any pair (all occupations zero)
+        EXX_CUDA(p, cudaEventRecord(p->row_done, s));
+        EXX_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->row_done, 0));
+        for (int r = 0; r < n_orb; ++r)
+            if (!copied[r])
+                EXX_CUDA(p, cudaMemcpyAsync(kpsi_host + static_cast<size_t>(r) * p->M, kpsi + static_cast<size_t>(r) * p->M,
+                                            p->M * sizeof(double), cudaMemcpyDeviceToHost, p->copy_stream));
+        EXX_CUDA(p, cudaEventRecord(p->copy_done, p->copy_stream));
+        EXX_CUDA(p, cudaStreamWaitEvent(s, p->copy_done, 0));
     }
     exchange_energy_kernel<<<1, 1024, 0, s>>>(p->e_mat, p->occ_dev, n_orb, p->ex_dev);
     EXX_CUDA(p, cudaGetLastError());
@@ -606,6 +629,9 @@ exx_status exx_plan_destroy(exx_plan* p) {
     if (p->occ_pinned) cudaFreeHost(p->occ_pinned);
     if (p->ex_pinned) cudaFreeHost(p->ex_pinned);
     if (p->upload_done) cudaEventDestroy(p->upload_done);
+    if (p->row_done) cudaEventDestroy(p->row_done);
+    if (p->copy_done) cudaEventDestroy(p->copy_done);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (cudaEvent_t ev : p->events) cudaEventDestroy(ev);
     if (p->psi_stage) cudaFree(p->psi_stage);
     if (p->kpsi_stage) cudaFree(p->kpsi_stage);
@@ -701,10 +727,14 @@ exx_status exx_apply_host(exx_plan* p, int n_orb, const double* psi_host, const 
         }
         p->stage_elems = elems;
     }
+    if (!p->copy_stream) {
+        EXX_CUDA(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        EXX_CUDA(p, cudaEventCreateWithFlags(&p->row_done, cudaEventDisableTiming));
+        EXX_CUDA(p, cudaEventCreateWithFlags(&p->copy_done, cudaEventDisableTiming));
+    }
     EXX_CUDA(p, cudaMemcpyAsync(p->psi_stage, psi_host, elems * sizeof(double), cudaMemcpyHostToDevice, p->stream));
-    st = apply_impl(p, n_orb, p->psi_stage, occ_host, p->kpsi_stage);
+    st = apply_impl(p, n_orb, p->psi_stage, occ_host, p->kpsi_stage, kpsi_host);
     if (st != EXX_OK) return st;
-    EXX_CUDA(p, cudaMemcpyAsync(kpsi_host, p->kpsi_stage, elems * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
     EXX_CUDA(p, cudaMemcpyAsync(p->ex_pinned, p->ex_dev, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
     *ex_host = *p->ex_pinned;
