@@ -80,6 +80,9 @@ def test_edge_cases_occupations_and_batching():
     ex_b = _check_full(w, occ=occ, symmetric=False, batch=1)
     ex_c = _check_full(w, occ=occ, symmetric=False, batch=2)
     assert abs(ex_a - ex_b) <= 1e-13 * abs(ex_a) and abs(ex_a - ex_c) <= 1e-13 * abs(ex_a)
+    # imaginary-slot-only transforms (f_j = f_i = 0, f_l != 0) and an even N with empty block-rows
+    w8 = make_workload(small_spec("C2", dims=(8, 16, 8), n_orb=8, number=76))
+    _check_full(w8, occ=[0.0, 1.2, 0.0, 0.0, 2.0, 0.0, 0.0, 0.7], symmetric=False, batch=3)
     # N = 1: Hartree special case
     w1 = make_workload(small_spec("C1", dims=(16, 16, 16), n_orb=1, number=78))
     _check_full(w1, occ=[1.3], symmetric=False)

@@ -65,20 +65,20 @@ CASES = [
 ]
 
 
-@pytest.mark.parametrize("ta,tb,tc,free,G,chunk", CASES)
-def test_emulated_batch_matches_oracle(emu, ta, tb, tc, free, G, chunk):
+def _run_case(emu, ta, tb, tc, free, G, chunk, n_orb, occ, max_batch=0):
+    """Runs the library's own schedule (exx_schedule_list) for these occupations through the emulated passes and
+    compares K psi and the pair energies with the oracle, pair by pair."""
+    import paper_1712_07973_b200 as exx
     dims = tuple(t // 2 if free else t for t in (ta, tb, tc))
     base = "C2" if free else "C1"
-    n_orb = 4 if max(ta, tb, tc) < 96 or min(ta, tb, tc) < 96 else 3
     w = make_workload(small_spec(base, dims=dims, n_orb=n_orb, spacing=(0.45, 0.5, 0.4), number=100 + ta + tb + tc))
     psi = np.ascontiguousarray(w["psi"].numpy())
     o = Oracle(dims, w["spec"].spacing, "free" if free else "periodic", w["kernel"])
-    occ = np.array([2.0, 1.5, 0.75, 1.0])[:n_orb]
-    # the same-(j,l) batch of block-row {0,1}: i = 0 carries only the diagonal pair (0,0); i = 1 the pairs (0,1), (1,1);
-    # i >= 2 the pairs (0,i), (1,i).  N = 3 cases also run the odd tail block-row {2} (l = -1).
-    batches = [(0, 1, [(i, 1 if i == 0 else 3) for i in range(n_orb)])]
-    if n_orb == 3:
-        batches.append((2, -1, [(2, 1)]))
+    occ = np.asarray(occ, dtype=np.float64)
+    rows = exx.exx_schedule_list(occ, max_batch)
+    batches = {}
+    for j, l, i, flags, b in rows.tolist():
+        batches.setdefault(b, (j, l, []))[2].append((i, flags))
     khat = o.khat()
     T_tot = ta * tb * tc
     ks = np.ascontiguousarray(khat.real[: ta // 2 + 1, : tb // 2 + 1, : tc // 2 + 1]) / T_tot
@@ -86,7 +86,8 @@ def test_emulated_batch_matches_oracle(emu, ta, tb, tc, free, G, chunk):
     twa, twc, rootsb = _tw(ta), _tw(tc), _roots(tb)
     d = lambda x: x.ctypes.data_as(C.POINTER(C.c_double))
     ref = np.zeros_like(psi)
-    for j, l, xf in batches:
+    for b in sorted(batches):
+        j, l, xf = batches[b]
         count = len(xf)
         iflags = np.array(xf, dtype=np.int32)
         fis = np.array([occ[i] for i, _ in xf])
@@ -108,6 +109,24 @@ def test_emulated_batch_matches_oracle(emu, ta, tb, tc, free, G, chunk):
                     ref[i] -= occ[x] * v * psi[x]
                 e_ref.append(np.sum(rho * v))
         e_ref = np.array(e_ref)
-        assert np.max(np.abs(e_out - e_ref)) <= 1e-12 * np.max(np.abs(e_ref))
-    scale = np.max(np.abs(ref))
+        assert np.max(np.abs(e_out - e_ref)) <= 1e-12 * max(np.max(np.abs(e_ref)), 1e-300)
+    # the batches together are the whole operator: compare with the oracle's definition as well
+    k_def, _, _ = o.apply(psi, occ, symmetric=False)
+    scale = np.max(np.abs(k_def))
+    assert np.max(np.abs(ref - k_def)) <= 1e-12 * scale
     assert np.max(np.abs(kpsi - ref)) <= 1e-12 * scale
+
+
+@pytest.mark.parametrize("ta,tb,tc,free,G,chunk", CASES)
+def test_emulated_batch_matches_oracle(emu, ta, tb, tc, free, G, chunk):
+    big = max(ta, tb, tc) >= 96 and min(ta, tb, tc) >= 96
+    n_orb = 3 if big else 4                              # N = 3: odd tail block-row {2} with l = -1
+    _run_case(emu, ta, tb, tc, free, G, chunk, n_orb, [2.0, 1.5, 0.75, 1.0][:n_orb])
+
+
+@pytest.mark.parametrize("occ,max_batch", [([0.0, 1.2, 0.0, 0.0, 2.0], 0),      # imaginary-slot-only transforms (flags = 2), odd N
+                                           ([2.0, 0.0, 1.0, 0.0, 0.0, 0.3], 2),  # real-slot-only transforms, block-rows cut in batches
+                                           ([1.0, 2.0, 0.5], 1)])                # one transform per batch: i = j and i = l alone
+def test_emulated_schedule_edge_cases(emu, occ, max_batch):
+    _run_case(emu, 16, 16, 16, 0, 2, 2, len(occ), occ, max_batch)
+    _run_case(emu, 16, 16, 16, 1, 2, 4, len(occ), occ, max_batch)
