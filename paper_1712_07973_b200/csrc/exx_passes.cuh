@@ -628,10 +628,12 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     for (int m = 0; m < NI2; ++m) c2[m] = col_index<C, false>(tid + m * NT < C::ITEMS_POS ? tid + m * NT : 0, a, b2base, g.na);
     const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
 
+    int flags_next = g.desc[0].flags;                          // descriptor of the next transform, one iteration ahead
     for (int t = 0; t < g.count; ++t) {
         const int s = t % NSTG;
         double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
-        const int flags = g.desc[t].flags;
+        const int flags = flags_next;
+        if (t + 1 < g.count) flags_next = g.desc[t + 1].flags;
         mbar_wait(&full[s], (t / NSTG) & 1);
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
@@ -831,11 +833,13 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         for (int n1 = 0; n1 < C::PCN; ++n1) { accj[m][n1] = 0.0; accl[m][n1] = 0.0; }
     }
 
+    XformDesc d_next = g.desc[0];                              // descriptor of the next transform, one iteration ahead
     for (int t = 0; t < g.count; ++t) {
         double2* S = S0 + (NBUF == 2 ? (t & 1) : 0) * C::SMEM_C;
         const int s = t % NSTG;
         double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
-        const XformDesc d = g.desc[t];
+        const XformDesc d = d_next;
+        if (t + 1 < g.count) d_next = g.desc[t + 1];
         if (NBUF == 2) {
             if (t + 1 < g.count) issue_w1_gather(t + 1);
             cp_async_commit();
