@@ -35,7 +35,7 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
     if constexpr (!T::FITS) {
         return cudaErrorInvalidValue;
     } else {
-        auto kern = pass_b_kernel<C, T::NT, T::MINB>;
+        auto kern = T::WS ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB> : pass_b_kernel<C, T::NT, T::MINB>;
         static bool done = false;
         static int occ = 0;
         if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; }
@@ -73,15 +73,6 @@ cudaError_t query_pass_b(const Geometry& g, KernelInfo* info) {
     args.npch = g.tc / g.chunk;
     return dispatch_b(g, args, 0, nullptr, info, false);
 }
-
-#ifdef EXX_DEBUG_TIMING
-extern "C" void exx_debug_b_read(long long* out16) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out16, g_dbg_b, sizeof(long long) * 16);
-    long long z[16] = {0};
-    cudaMemcpyToSymbol(g_dbg_b, z, sizeof(z));
-}
-#endif
 
 bool length_supported(int t) {
     return t == 16 || t == 32 || t == 64 || t == 96 || t == 128 || t == 192 || t == 256;

@@ -654,12 +654,6 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     }
 }
 
-#ifdef EXX_DEBUG_TIMING
-static __device__ long long g_dbg_b[16];
-#define EXX_DBG(k) do { if (dbg_on) { const long long now = clock64(); dbg_acc[k] += now - dbg_prev; dbg_prev = now; } } while (0)
-#else
-#define EXX_DBG(k) do { } while (0)
-#endif
 
 // Pass B.  Persistent CTAs over the (pch, q, t) blocks of the launch, t fastest (CTAs that run at the same time
 // share a K^ slice in L2).  The next block lands in a separate buffer by TMA bulk row copies while the current one is
@@ -699,28 +693,19 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
     };
     if (tid < 32 && static_cast<int>(blockIdx.x) < g.ntiles) issue_block_load(blockIdx.x);
 
-#ifdef EXX_DEBUG_TIMING
-    const bool dbg_on = tid == 0 || tid == NT - 32;
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long dbg_prev = clock64();
-#endif
     int it = 0;
     for (int id = blockIdx.x; id < g.ntiles; id += gridDim.x, ++it) {
         const int rest = id / g.count;
         const int q = rest % C::R1, pch = rest / C::R1;
         double2* blk = block_ptr(id);
-        EXX_DBG(6);
         mbar_wait(&full, it & 1);
-        EXX_DBG(0);
 #pragma unroll
         for (int m = 0; m < NIO; ++m)
             if (tid + m * NT < C::ITEMS_IO) {
                 const IoIdx x = io_index<C>(tid + m * NT);
                 b0_compute<C>(L + x.l, W + x.s);
             }
-        EXX_DBG(1);
         __syncthreads();
-        EXX_DBG(2);
         if (tid < 32 && id + static_cast<int>(gridDim.x) < g.ntiles) issue_block_load(id + gridDim.x);
         for (int cg = wid; cg < C::NGRP; cg += NW) {
 #pragma unroll
@@ -744,21 +729,148 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
             for (int m = 0; m < NQ; ++m)
                 if (lane + m * 32 < C::ITEMS_Q) b3_compute<C>(W + colq_index<C>(cg, lane + m * 32).base);
         }
-        EXX_DBG(3);
         __syncthreads();
-        EXX_DBG(4);
 #pragma unroll
         for (int m = 0; m < NIO; ++m)
             if (tid + m * NT < C::ITEMS_IO) {
                 const IoIdx x = io_index<C>(tid + m * NT);
                 b4_compute<C>(W + x.s, blk + x.g);
             }
-        EXX_DBG(5);
     }
-#ifdef EXX_DEBUG_TIMING
-    if (dbg_on)
-        for (int k = 0; k < 8; ++k) atomicAdd(reinterpret_cast<unsigned long long*>(&g_dbg_b[(tid == 0 ? 0 : 8) + k]), static_cast<unsigned long long>(dbg_acc[k]));
-#endif
+}
+
+// Pass B, warp-specialised variant (used where two work buffers fit shared memory: the periodic geometries).
+// NY "column" warps run the a-axis phases B1..B3 of block k while NX "row" warps run the b-axis phases of its
+// neighbours -- B0 of block k+1 in place in the OTHER buffer as soon as it has landed, B4 of block k-1 out of that
+// buffer before -- so the FP64-heavy and the load/store-heavy halves of the pass overlap inside one CTA.  There is no
+// CTA-wide barrier: blocks are handed over with mbarriers
+//     full[b]   TMA rows of a block have landed in buf[b] (straight into the padded work layout)   -> row warps
+//     ready[b]  B0 done on buf[b]  (row warps arrive)                                                -> column warps
+//     done[b]   B1..B3 done on buf[b] (column warps arrive)                                          -> row warps
+// and the row warps refill buf[b] with block k+2 once B4 of block k has drained it.
+template <class C, int NY, int NX, int MINB>
+__global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const ArgsB g) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* const BUF = reinterpret_cast<double2*>(smem_raw);           // two buffers of WORK_ELEMS
+    double2* const TW1 = BUF + 2 * C::WORK_ELEMS;
+    double2* const TW2 = TW1 + C::TA;
+    __shared__ uint64_t full[2], ready[2], done[2];
+    constexpr int NT = 32 * (NY + NX), NXT = 32 * NX;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    constexpr int NQ = ceil_div(C::ITEMS_Q, 32), NP = ceil_div(C::ITEMS_P, 32), NIO = ceil_div(C::ITEMS_IO, NXT);
+
+    if (tid == 0) {
+        for (int b = 0; b < 2; ++b) { mbar_init(&full[b], NX); mbar_init(&ready[b], NX); mbar_init(&done[b], NY); }
+        mbar_fence_init();
+    }
+    for (int x = tid; x < C::TA; x += NT) {
+        const double2 v = g.twa[x];
+        TW1[x] = v;
+        TW2[(x % C::QA) * C::PA + x / C::QA] = v;
+    }
+    __syncthreads();
+    auto block_ptr = [&](int id) -> double2* {             // id -> (pch, q, t), t fastest
+        const int t = id % g.count, rest = id / g.count;
+        const int q = rest % C::R1, pch = rest / C::R1;
+        return g.w1 + ((static_cast<size_t>(t) * C::R1 + q) * g.npch + pch) * C::BLOCK_ELEMS;
+    };
+    const int stride = gridDim.x, id0 = blockIdx.x;
+    const int nk = id0 < g.ntiles ? (g.ntiles - id0 + stride - 1) / stride : 0;
+
+    if (wid >= NY) {
+        // ------------------------------------------------------------------ row warps: landing, B0, B4, refill
+        // A row warp owns the rows a of its (a, pin) items for the whole kernel: it alone reads and writes them in B0
+        // and B4, and it alone refills them, so the row warps never wait for one another.
+        const int xt = tid - 32 * NY;
+        int my_rows = 0;                                   // rows this warp refills (for the transaction count)
+#pragma unroll
+        for (int m = 0; m < NIO; ++m) {
+            const int first = (xt - lane) + m * NXT;       // first item of this warp in round m
+            const int n_items = C::ITEMS_IO - first < 32 ? C::ITEMS_IO - first : 32;
+            if (n_items > 0) my_rows += (n_items + C::CHUNK - 1) / C::CHUNK;
+        }
+        auto issue_row_loads = [&](int k) {                // all lanes of this warp
+            const double2* src = block_ptr(id0 + k * stride);
+            double2* dst = BUF + (k & 1) * C::WORK_ELEMS;
+            if (lane == 0) mbar_arrive_expect_tx(&full[k & 1], my_rows * C::ROW_BYTES);
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < NIO; ++m) {
+                const int idx = xt + m * NXT;
+                if (idx < C::ITEMS_IO && idx % C::CHUNK == 0) {
+                    const int a = idx / C::CHUNK;
+                    bulk_g2s(dst + C::row_off(a), src + a * C::COLS, C::ROW_BYTES, &full[k & 1]);
+                }
+            }
+        };
+        auto b4_block = [&](int k) {
+            double2* const W = BUF + (k & 1) * C::WORK_ELEMS;
+            double2* blk = block_ptr(id0 + k * stride);
+            mbar_wait(&done[k & 1], (k >> 1) & 1);
+#pragma unroll
+            for (int m = 0; m < NIO; ++m)
+                if (xt + m * NXT < C::ITEMS_IO) {
+                    const IoIdx x = io_index<C>(xt + m * NXT);
+                    b4_compute<C>(W + x.s, blk + x.g);
+                }
+        };
+        if (nk > 0) issue_row_loads(0);
+        if (nk > 1) issue_row_loads(1);
+        for (int k = 0; k < nk; ++k) {
+            double2* const W = BUF + (k & 1) * C::WORK_ELEMS;
+            mbar_wait(&full[k & 1], (k >> 1) & 1);
+#pragma unroll
+            for (int m = 0; m < NIO; ++m)
+                if (xt + m * NXT < C::ITEMS_IO) {
+                    const IoIdx x = io_index<C>(xt + m * NXT);
+                    b0_compute<C>(W + x.s, W + x.s);       // in place
+                }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&ready[k & 1]);
+            if (k >= 1) {
+                b4_block(k - 1);
+                if (k + 1 < nk) {
+                    fence_proxy_async();                   // this warp's reads of its rows precede the TMA writes
+                    __syncwarp();
+                    issue_row_loads(k + 1);
+                }
+            }
+        }
+        if (nk > 0) b4_block(nk - 1);
+    } else {
+        // ------------------------------------------------------------------ column warps: a-axis phases
+        for (int k = 0; k < nk; ++k) {
+            const int id = id0 + k * stride;
+            double2* const W = BUF + (k & 1) * C::WORK_ELEMS;
+            const int rest = id / g.count;
+            const int q = rest % C::R1, pch = rest / C::R1;
+            mbar_wait(&ready[k & 1], (k >> 1) & 1);
+            for (int cg = wid; cg < C::NGRP; cg += NY) {
+#pragma unroll
+                for (int m = 0; m < NQ; ++m)
+                    if (lane + m * 32 < C::ITEMS_Q) {
+                        const ColAIdx x = colq_index<C>(cg, lane + m * 32);
+                        b1_compute<C>(W + x.base, TW1 + x.k, C::QA);
+                    }
+                __syncwarp();
+#pragma unroll
+                for (int m = 0; m < NP; ++m)
+                    if (lane + m * 32 < C::ITEMS_P) {
+                        const ColAIdx x = colp_index<C>(cg, lane + m * 32);
+                        const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
+                        const int kb = q + C::R1 * r;
+                        const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
+                        b2_compute<C>(W + x.base, g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA, TW2 + x.k, C::PA, x.k);
+                    }
+                __syncwarp();
+#pragma unroll
+                for (int m = 0; m < NQ; ++m)
+                    if (lane + m * 32 < C::ITEMS_Q) b3_compute<C>(W + colq_index<C>(cg, lane + m * 32).base);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&done[k & 1]);
+        }
+    }
 }
 
 // Pass C.  One CTA per (a, b2-group) tile; it loops over the transforms of the same-(j,l) batch, keeps the K psi_j and
