@@ -113,15 +113,19 @@ struct TuneAC {
 template <int TA, int TB, bool FREE, int CHUNK>
 struct TuneB {
     using Cfg = CfgB<TA, TB, FREE, CHUNK>;
-    // warp-specialised variant (two full work buffers, column warps + row warps) where it fits and the block is big
-    // enough to feed both kinds of warps; else work + landing buffer with CTA barriers
-    static constexpr int SMEM_WS = (2 * Cfg::WORK_ELEMS + 2 * TA) * 16;
+    // warp-specialised variant (column warps + row warps, two block buffers) where it fits and the block is big enough
+    // to feed both kinds of warps: WS with two full work buffers, else (free BC) WSF with NA-row buffers and per-warp
+    // expansion scratch; else work + landing buffer with CTA barriers
     static constexpr int NY = Cfg::NGRP <= 12 ? Cfg::NGRP : Cfg::NGRP / 2;       // column warps
     static constexpr int NX = 4;                                                // row warps
-    static constexpr bool WS = SMEM_WS <= kMaxSmemB && Cfg::NGRP >= 6 && (Cfg::NGRP <= 12 || Cfg::NGRP % 2 == 0);
-    static constexpr int SMEM = WS ? SMEM_WS : Cfg::SMEM_BYTES;
+    static constexpr bool kBig = Cfg::NGRP >= 6 && (Cfg::NGRP <= 12 || Cfg::NGRP % 2 == 0);
+    static constexpr int SMEM_WS = (2 * Cfg::WORK_ELEMS + 2 * TA) * 16;
+    static constexpr int SMEM_WSF = (2 * Cfg::P_ELEMS + NY * Cfg::E_ELEMS + 2 * TA) * 16;
+    static constexpr bool WS = kBig && SMEM_WS <= kMaxSmemB;
+    static constexpr bool WSF = kBig && !WS && FREE && SMEM_WSF <= kMaxSmemB;
+    static constexpr int SMEM = WS ? SMEM_WS : WSF ? SMEM_WSF : Cfg::SMEM_BYTES;
     // one warp per column group, at most 16 warps; small blocks share an SM (persistent grid = SMs * MINB)
-    static constexpr int NT = WS ? 32 * (NY + NX) : 32 * imin(Cfg::NGRP, 16);
+    static constexpr int NT = (WS || WSF) ? 32 * (NY + NX) : 32 * imin(Cfg::NGRP, 16);
     static constexpr int MINB = imax(1, imin(imin(kSmemPerSM / (SMEM + 1024), 512 / NT), 8));
     static constexpr bool FITS = SMEM <= kMaxSmemB;
 };

@@ -35,7 +35,8 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
     if constexpr (!T::FITS) {
         return cudaErrorInvalidValue;
     } else {
-        auto kern = T::WS ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB> : pass_b_kernel<C, T::NT, T::MINB>;
+        auto kern = T::WS ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB, false>
+                  : T::WSF ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB, true> : pass_b_kernel<C, T::NT, T::MINB>;
         static bool done = false;
         static int occ = 0;
         if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; }

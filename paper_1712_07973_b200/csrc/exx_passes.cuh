@@ -422,6 +422,18 @@ constexpr int chunk_for(int ta, int tb, bool free_bc) {
     return smem_b_bytes(ta, tb, free_bc, 4) <= kMaxSmemB ? 4 : smem_b_bytes(ta, tb, free_bc, 2) <= kMaxSmemB ? 2 : 1;
 }
 
+// skew between the k1-blocks of the expansion scratch: B2's lanes (k1 = lane / NCW, cw = lane % NCW) must not collide
+constexpr int pick_pade(int qa, int pa, int ncw) {
+    int best = 0, best_cost = 1 << 30;
+    for (int pad = 0; pad < 8; ++pad) {
+        int o[32] = {};
+        for (int l = 0; l < 32; ++l) o[l] = (l / ncw) * (qa * ncw + pad) + l % ncw;
+        const int c = wavefronts32(o, pa * ncw < 32 ? pa * ncw : 32) * 16 + pad;
+        if (c < best_cost) { best_cost = c; best = pad; }
+    }
+    return best;
+}
+
 template <int TA_, int TB_, bool FREE_, int CHUNK_>
 struct CfgB {
     static constexpr int TA = TA_, TB = TB_, CHUNK = CHUNK_;
@@ -447,6 +459,11 @@ struct CfgB {
     static constexpr int NSA = TA / 2 + 1;                 // symmetric a-range of K^
     static constexpr int SMEM_BYTES = (WORK_ELEMS + LAND_ELEMS + 2 * TA) * 16;
     EXX_HD static int row_off(int a) { return (a / QA) * QRS + (a % QA) * RS; }
+    // warp-private expansion scratch of the free-BC warp-specialised variant: the TA rows of the NCW columns a warp
+    // owns, element (row k1*QA + n2, column cw) at k1*QRSE + n2*NCW + cw; the block buffers then hold NA rows only
+    static constexpr int QRSE = QA * NCW + pick_pade(QA, PA, NCW);
+    static constexpr int E_ELEMS = PA * QRSE;
+    static constexpr int P_ELEMS = PAN * QRS;              // block buffer with the NA rows that exist in W1
 };
 
 struct ArgsB {
@@ -561,6 +578,53 @@ EXX_HD void b4_compute(const double2* src, double2* dst) {
     dft_inv<C::R2, false>(xr, xi);
 #pragma unroll
     for (int b2 = 0; b2 < C::R2; ++b2) dst[b2 * C::CHUNK] = make_double2(xr[b2], xi[b2]);
+}
+
+// ---- free-BC variants with the expansion scratch E (warp-private, see CfgB::QRSE): B1 block buffer -> E, B2 in E,
+//      B3 E -> block buffer.  in / out point at the item's first element; strides as in the in-place versions.
+template <class C>
+EXX_HD void b1e_compute(const double2* in, double2* out, const double2* tw, int tws) {
+    double xr[C::PA], xi[C::PA];
+#pragma unroll
+    for (int n1 = 0; n1 < C::PAN; ++n1) { double2 v = in[n1 * C::QRS]; xr[n1] = v.x; xi[n1] = v.y; }
+#pragma unroll
+    for (int n1 = C::PAN; n1 < C::PA; ++n1) { xr[n1] = 0.0; xi[n1] = 0.0; }
+    dft_fwd<C::PA, C::FREE>(xr, xi);
+#pragma unroll
+    for (int k1 = 0; k1 < C::PA; ++k1) {
+        if (k1 > 0) cmul(xr[k1], xi[k1], tw[k1 * tws]);
+        out[k1 * C::QRSE] = make_double2(xr[k1], xi[k1]);
+    }
+}
+template <class C>
+EXX_HD void b2e_compute(double2* colp, const double* kcol, const double2* tw, int tws, int k1) {
+    double xr[C::QA], xi[C::QA];
+    double kv[C::QA];
+#pragma unroll
+    for (int k2 = 0; k2 < C::QA; ++k2) {
+        const int ka = k1 + C::PA * k2;
+        kv[k2] = ld_ro(kcol + (ka <= C::TA - ka ? ka : C::TA - ka));
+    }
+#pragma unroll
+    for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = colp[n2 * C::NCW]; xr[n2] = v.x; xi[n2] = v.y; }
+    Dft<C::QA>::run(xr, xi);
+#pragma unroll
+    for (int k2 = 0; k2 < C::QA; ++k2) { xr[k2] *= kv[k2]; xi[k2] *= kv[k2]; }
+    dft_inv<C::QA, false>(xr, xi);
+#pragma unroll
+    for (int n2 = 0; n2 < C::QA; ++n2) {
+        if (k1 > 0) cmul_conj(xr[n2], xi[n2], tw[n2 * tws]);
+        colp[n2 * C::NCW] = make_double2(xr[n2], xi[n2]);
+    }
+}
+template <class C>
+EXX_HD void b3e_compute(const double2* in, double2* out) {
+    double xr[C::PA], xi[C::PA];
+#pragma unroll
+    for (int k1 = 0; k1 < C::PA; ++k1) { double2 v = in[k1 * C::QRSE]; xr[k1] = v.x; xi[k1] = v.y; }
+    dft_inv<C::PA, C::FREE>(xr, xi);
+#pragma unroll
+    for (int n1 = 0; n1 < C::PAN; ++n1) out[n1 * C::QRS] = make_double2(xr[n1], xi[n1]);
 }
 
 // ---------------------------------------------------------------------------------------- kernels
@@ -748,11 +812,16 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
 //     ready[b]  B0 done on buf[b]  (row warps arrive)                                                -> column warps
 //     done[b]   B1..B3 done on buf[b] (column warps arrive)                                          -> row warps
 // and the row warps refill buf[b] with block k+2 once B4 of block k has drained it.
-template <class C, int NY, int NX, int MINB>
+// SCRATCH (free BC, where two TA-row buffers do not fit): the block buffers hold only the NA rows that exist in W1 and
+// every column warp expands its NCW columns to TA rows in a private scratch (B1 buffer -> scratch, B2 in the scratch,
+// B3 scratch -> buffer).
+template <class C, int NY, int NX, int MINB, bool SCRATCH>
 __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const ArgsB g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2* const BUF = reinterpret_cast<double2*>(smem_raw);           // two buffers of WORK_ELEMS
-    double2* const TW1 = BUF + 2 * C::WORK_ELEMS;
+    constexpr int BUF_ELEMS = SCRATCH ? C::P_ELEMS : C::WORK_ELEMS;
+    double2* const BUF = reinterpret_cast<double2*>(smem_raw);           // two block buffers
+    double2* const ESC = BUF + 2 * BUF_ELEMS;                            // NY scratch areas (SCRATCH only)
+    double2* const TW1 = ESC + (SCRATCH ? NY * C::E_ELEMS : 0);
     double2* const TW2 = TW1 + C::TA;
     __shared__ uint64_t full[2], ready[2], done[2];
     constexpr int NT = 32 * (NY + NX), NXT = 32 * NX;
@@ -791,7 +860,7 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
         }
         auto issue_row_loads = [&](int k) {                // all lanes of this warp
             const double2* src = block_ptr(id0 + k * stride);
-            double2* dst = BUF + (k & 1) * C::WORK_ELEMS;
+            double2* dst = BUF + (k & 1) * BUF_ELEMS;
             if (lane == 0) mbar_arrive_expect_tx(&full[k & 1], my_rows * C::ROW_BYTES);
             __syncwarp();
 #pragma unroll
@@ -804,7 +873,7 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
             }
         };
         auto b4_block = [&](int k) {
-            double2* const W = BUF + (k & 1) * C::WORK_ELEMS;
+            double2* const W = BUF + (k & 1) * BUF_ELEMS;
             double2* blk = block_ptr(id0 + k * stride);
             mbar_wait(&done[k & 1], (k >> 1) & 1);
 #pragma unroll
@@ -817,7 +886,7 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
         if (nk > 0) issue_row_loads(0);
         if (nk > 1) issue_row_loads(1);
         for (int k = 0; k < nk; ++k) {
-            double2* const W = BUF + (k & 1) * C::WORK_ELEMS;
+            double2* const W = BUF + (k & 1) * BUF_ELEMS;
             mbar_wait(&full[k & 1], (k >> 1) & 1);
 #pragma unroll
             for (int m = 0; m < NIO; ++m)
@@ -841,31 +910,43 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
         // ------------------------------------------------------------------ column warps: a-axis phases
         for (int k = 0; k < nk; ++k) {
             const int id = id0 + k * stride;
-            double2* const W = BUF + (k & 1) * C::WORK_ELEMS;
+            double2* const W = BUF + (k & 1) * BUF_ELEMS;
             const int rest = id / g.count;
             const int q = rest % C::R1, pch = rest / C::R1;
             mbar_wait(&ready[k & 1], (k >> 1) & 1);
             for (int cg = wid; cg < C::NGRP; cg += NY) {
+                double2* const E = ESC + wid * C::E_ELEMS;
 #pragma unroll
                 for (int m = 0; m < NQ; ++m)
                     if (lane + m * 32 < C::ITEMS_Q) {
-                        const ColAIdx x = colq_index<C>(cg, lane + m * 32);
-                        b1_compute<C>(W + x.base, TW1 + x.k, C::QA);
+                        const int w = lane + m * 32;
+                        const ColAIdx x = colq_index<C>(cg, w);
+                        if (SCRATCH) b1e_compute<C>(W + x.base, E + w, TW1 + x.k, C::QA);     // E offset n2*NCW + cw = w
+                        else b1_compute<C>(W + x.base, TW1 + x.k, C::QA);
                     }
                 __syncwarp();
 #pragma unroll
                 for (int m = 0; m < NP; ++m)
                     if (lane + m * 32 < C::ITEMS_P) {
-                        const ColAIdx x = colp_index<C>(cg, lane + m * 32);
+                        const int w = lane + m * 32;
+                        const ColAIdx x = colp_index<C>(cg, w);
                         const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
                         const int kb = q + C::R1 * r;
                         const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-                        b2_compute<C>(W + x.base, g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA, TW2 + x.k, C::PA, x.k);
+                        const double* kcol = g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA;
+                        if (SCRATCH) b2e_compute<C>(E + x.k * C::QRSE + w % C::NCW, kcol, TW2 + x.k, C::PA, x.k);
+                        else b2_compute<C>(W + x.base, kcol, TW2 + x.k, C::PA, x.k);
                     }
                 __syncwarp();
 #pragma unroll
                 for (int m = 0; m < NQ; ++m)
-                    if (lane + m * 32 < C::ITEMS_Q) b3_compute<C>(W + colq_index<C>(cg, lane + m * 32).base);
+                    if (lane + m * 32 < C::ITEMS_Q) {
+                        const int w = lane + m * 32;
+                        const ColAIdx x = colq_index<C>(cg, w);
+                        if (SCRATCH) b3e_compute<C>(E + w, W + x.base);
+                        else b3_compute<C>(W + x.base);
+                    }
+                if (SCRATCH) __syncwarp();                 // the scratch is reused by this warp's next column group
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&done[k & 1]);

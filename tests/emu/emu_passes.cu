@@ -11,7 +11,7 @@
 using namespace exx;
 
 template <int TA, int TB, int TC, bool FREE, int G, int CHUNK>
-static int emu_batch(const double* psi, double* kpsi, int j, int l, double fj, double fl, int count, const XformDesc* desc,
+static int emu_batch(bool scratch, const double* psi, double* kpsi, int j, int l, double fj, double fl, int count, const XformDesc* desc,
                      const double2* twa, const double2* twc, const double2* rootsb, const double* ks_sym,
                      double* e_out /*[count][2]*/) {
     using AC = CfgAC<TC, TB, FREE, G, CHUNK>;
@@ -39,7 +39,7 @@ static int emu_batch(const double* psi, double* kpsi, int j, int l, double fj, d
     g.psi = psi; g.kpsi = kpsi; g.w1 = w1.data(); g.desc = desc; g.twc = twc; g.twb = twb.data();
     g.m_points = m_points; g.na = na; g.j = j; g.l = l; g.fj = fj; g.fl = fl; g.count = count;
     const size_t qstride = AC::w1_q(na), tstride = AC::w1_t(na);
-    std::vector<double2> S(AC::SMEM_A), SC(AC::SMEM_C), W(B::WORK_ELEMS), L(B::LAND_ELEMS);
+    std::vector<double2> S(AC::SMEM_A), SC(AC::SMEM_C), W(B::WORK_ELEMS), L(B::LAND_ELEMS), E(B::E_ELEMS);
     std::vector<double> op(AC::OP_DOUBLES), res(AC::RES_DOUBLES);
     std::vector<double> vj(static_cast<size_t>(AC::ITEMS_LINE_Q) * AC::PCN), vl(vj.size()), accj(vj.size()), accl(vj.size());
     auto stage_lines = [&](int orb, double* dst, int a, int b2base) {       // the kernels' TMA bulk line loads
@@ -77,19 +77,38 @@ static int emu_batch(const double* psi, double* kpsi, int j, int l, double fj, d
         const int q = id % B::R1, pch = (id / B::R1) % npch, t = id / (B::R1 * npch);
         double2* blk = w1.data() + ((static_cast<size_t>(t) * B::R1 + q) * npch + pch) * B::BLOCK_ELEMS;
         for (int a = 0; a < B::NA; ++a) std::memcpy(&L[a * B::RSL], blk + a * B::COLS, B::ROW_BYTES);   // TMA bulk row loads
-        for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b0_compute<B>(L.data() + x.l, W.data() + x.s); }
-        for (int cg = 0; cg < B::NGRP; ++cg) {
-            for (int w = 0; w < B::ITEMS_Q; ++w) { const ColAIdx x = colq_index<B>(cg, w); b1_compute<B>(W.data() + x.base, twa + x.k, B::QA); }
-            for (int w = 0; w < B::ITEMS_P; ++w) {
-                const ColAIdx x = colp_index<B>(cg, w);
-                const int r = x.col / CHUNK, pin = x.col % CHUNK;
-                const int kb = q + B::R1 * r;
-                const int sb = kb <= TB - kb ? kb : TB - kb;
-                b2_compute<B>(W.data() + x.base, ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, twa2.data() + x.k, B::PA, x.k);
+        if (!scratch) {
+            for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b0_compute<B>(L.data() + x.l, W.data() + x.s); }
+            for (int cg = 0; cg < B::NGRP; ++cg) {
+                for (int w = 0; w < B::ITEMS_Q; ++w) { const ColAIdx x = colq_index<B>(cg, w); b1_compute<B>(W.data() + x.base, twa + x.k, B::QA); }
+                for (int w = 0; w < B::ITEMS_P; ++w) {
+                    const ColAIdx x = colp_index<B>(cg, w);
+                    const int r = x.col / CHUNK, pin = x.col % CHUNK;
+                    const int kb = q + B::R1 * r;
+                    const int sb = kb <= TB - kb ? kb : TB - kb;
+                    b2_compute<B>(W.data() + x.base, ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, twa2.data() + x.k, B::PA, x.k);
+                }
+                for (int w = 0; w < B::ITEMS_Q; ++w) b3_compute<B>(W.data() + colq_index<B>(cg, w).base);
             }
-            for (int w = 0; w < B::ITEMS_Q; ++w) b3_compute<B>(W.data() + colq_index<B>(cg, w).base);
+            for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b4_compute<B>(W.data() + x.s, blk + x.g); }
+        } else {
+            // the warp-specialised kernels: the block lands straight in the padded layout, B0 in place; with the free-BC
+            // expansion scratch the buffer holds NA rows and every column group expands into E
+            for (int a = 0; a < B::NA; ++a) std::memcpy(&W[B::row_off(a)], blk + a * B::COLS, B::ROW_BYTES);
+            for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b0_compute<B>(W.data() + x.s, W.data() + x.s); }
+            for (int cg = 0; cg < B::NGRP; ++cg) {
+                for (int w = 0; w < B::ITEMS_Q; ++w) { const ColAIdx x = colq_index<B>(cg, w); b1e_compute<B>(W.data() + x.base, E.data() + w, twa + x.k, B::QA); }
+                for (int w = 0; w < B::ITEMS_P; ++w) {
+                    const ColAIdx x = colp_index<B>(cg, w);
+                    const int r = x.col / CHUNK, pin = x.col % CHUNK;
+                    const int kb = q + B::R1 * r;
+                    const int sb = kb <= TB - kb ? kb : TB - kb;
+                    b2e_compute<B>(E.data() + x.k * B::QRSE + w % B::NCW, ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, twa2.data() + x.k, B::PA, x.k);
+                }
+                for (int w = 0; w < B::ITEMS_Q; ++w) b3e_compute<B>(E.data() + w, W.data() + colq_index<B>(cg, w).base);
+            }
+            for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b4_compute<B>(W.data() + x.s, blk + x.g); }
         }
-        for (int w = 0; w < B::ITEMS_IO; ++w) { const IoIdx x = io_index<B>(w); b4_compute<B>(W.data() + x.s, blk + x.g); }
     }
     // pass C: the W1 columns land in place in the work buffer (the kernel's cp.async gather); psi_j / psi_l lines are
     // resident, the psi_i lines are staged in an operand buffer that C2 overwrites with the K psi_i increment (the
@@ -141,9 +160,11 @@ static int emu_batch(const double* psi, double* kpsi, int j, int l, double fj, d
 
 #define EMU_CASE(TA_, TB_, TC_, FREE_, G_, CH_)                                                              \
     if (ta == TA_ && tb == TB_ && tc == TC_ && free_bc == FREE_ && g == G_ && chunk == CH_)                    \
-        return emu_batch<TA_, TB_, TC_, FREE_ != 0, G_, CH_>(psi, kpsi, j, l, fj, fl, count, desc, twa, twc, rootsb, ks, e_out);
+        return emu_batch<TA_, TB_, TC_, FREE_ != 0, G_, CH_>(variant != 0, psi, kpsi, j, l, fj, fl, count, desc, twa, twc, rootsb, ks, e_out);
 
-extern "C" int exx_emu_batch(int ta, int tb, int tc, int free_bc, int g, int chunk, const double* psi, double* kpsi,
+// variant 0: pass B with landing + work buffer (pass_b_kernel); 1: in-place landing with the expansion scratch
+// (pass_b_ws_kernel<SCRATCH>; for periodic grids the scratch path is still a valid evaluation order)
+extern "C" int exx_emu_batch(int variant, int ta, int tb, int tc, int free_bc, int g, int chunk, const double* psi, double* kpsi,
                              int j, int l, double fj, double fl, int count, const int* iflags /*[count][2]*/,
                              const double* fis /*[count]*/, const double* twa_, const double* twc_, const double* rootsb_,
                              const double* ks, double* e_out) {

@@ -41,7 +41,7 @@ def _build():
 def emu():
     lib = C.CDLL(_build())
     dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int)
-    lib.exx_emu_batch.argtypes = [C.c_int] * 6 + [dp, dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, ip, dp, dp, dp, dp, dp, dp]
+    lib.exx_emu_batch.argtypes = [C.c_int] * 7 + [dp, dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, ip, dp, dp, dp, dp, dp, dp]
     return lib
 
 
@@ -65,7 +65,7 @@ CASES = [
 ]
 
 
-def _run_case(emu, ta, tb, tc, free, G, chunk, n_orb, occ, max_batch=0):
+def _run_case(emu, ta, tb, tc, free, G, chunk, n_orb, occ, max_batch=0, variant=0):
     """Runs the library's own schedule (exx_schedule_list) for these occupations through the emulated passes and
     compares K psi and the pair energies with the oracle, pair by pair."""
     import paper_1712_07973_b200 as exx
@@ -92,7 +92,7 @@ def _run_case(emu, ta, tb, tc, free, G, chunk, n_orb, occ, max_batch=0):
         iflags = np.array(xf, dtype=np.int32)
         fis = np.array([occ[i] for i, _ in xf])
         e_out = np.zeros(2 * count)
-        rc = emu.exx_emu_batch(ta, tb, tc, free, G, chunk, d(psi), d(kpsi), j, l, float(occ[j]), float(occ[l]) if l >= 0 else 0.0,
+        rc = emu.exx_emu_batch(variant, ta, tb, tc, free, G, chunk, d(psi), d(kpsi), j, l, float(occ[j]), float(occ[l]) if l >= 0 else 0.0,
                                count, iflags.ctypes.data_as(C.POINTER(C.c_int)), d(fis), d(twa.view(np.float64)),
                                d(twc.view(np.float64)), d(rootsb.view(np.float64)), d(ks), d(e_out))
         assert rc == 0, "case not instantiated in tests/emu/emu_passes.cu"
@@ -122,6 +122,12 @@ def test_emulated_batch_matches_oracle(emu, ta, tb, tc, free, G, chunk):
     big = max(ta, tb, tc) >= 96 and min(ta, tb, tc) >= 96
     n_orb = 3 if big else 4                              # N = 3: odd tail block-row {2} with l = -1
     _run_case(emu, ta, tb, tc, free, G, chunk, n_orb, [2.0, 1.5, 0.75, 1.0][:n_orb])
+
+
+@pytest.mark.parametrize("ta,tb,tc,free,G,chunk", [c for c in CASES if c[3] == 1][:6] + [(32, 32, 32, 0, 4, 4)])
+def test_emulated_scratch_variant_matches_oracle(emu, ta, tb, tc, free, G, chunk):
+    """The warp-specialised pass B: block landed in place, a-axis phases through the per-warp expansion scratch."""
+    _run_case(emu, ta, tb, tc, free, G, chunk, 3, [2.0, 1.5, 0.75], variant=1)
 
 
 @pytest.mark.parametrize("occ,max_batch", [([0.0, 1.2, 0.0, 0.0, 2.0], 0),      # imaginary-slot-only transforms (flags = 2), odd N
