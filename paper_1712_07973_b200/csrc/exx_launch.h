@@ -126,7 +126,7 @@ struct TuneB {
     static constexpr int SMEM = WS ? SMEM_WS : WSF ? SMEM_WSF : Cfg::SMEM_BYTES;
     // one warp per column group, at most 16 warps; small blocks share an SM (persistent grid = SMs * MINB)
     static constexpr int NT = (WS || WSF) ? 32 * (NY + NX) : 32 * imin(Cfg::NGRP, 16);
-    static constexpr int MINB = imax(1, imin(imin(kSmemPerSM / (SMEM + 1024), 512 / NT), 8));
+    static constexpr int MINB = imax(1, imin(imin(kSmemPerSM / (SMEM + 1024), imax(1, 512 / NT)), 8));
     static constexpr bool FITS = SMEM <= kMaxSmemB;
 };
 
