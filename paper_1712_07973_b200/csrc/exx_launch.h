@@ -107,7 +107,17 @@ struct TuneAC {
     static constexpr int NSTG_A = 2;
     static constexpr int SMEM_A = smem_ac_bytes<TC, TB, FREE>(G_A, NSTG_A, false);
     static constexpr int MINB_A = pick_minb(SMEM_A + (TC + TB) * 16 + 64, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
-    static_assert(SMEM_C <= kMaxSmemAC && SMEM_A <= kMaxSmemAC, "tile does not fit shared memory");
+    // ---- pass A, warp-specialised (lengths >= 96): line warps for A0/A1, column warps for A2, two work buffers
+    static constexpr bool WS_A = TC >= 96;
+    static constexpr int NAW = imin(6, imax(1, (imax(CfgA::ITEMS_LINE_Q, CfgA::ITEMS_LINE_P) + 31) / 32));
+    static constexpr int NBW = imax(2, 8 - NAW);
+    static constexpr int kStaticA = (TC + TB) * 16 + 128;
+    static constexpr int NSTG_A_WS =                       // one operand stage if that is what lets two CTAs share an SM
+        (2 * CfgA::SMEM_A * 16 + 2 * CfgA::OP_DOUBLES * 8 + kStaticA) * 2 <= kSmemPerSM + 1024 ? 2 :
+        (2 * CfgA::SMEM_A * 16 + 1 * CfgA::OP_DOUBLES * 8 + kStaticA) * 2 <= kSmemPerSM + 1024 ? 1 : 2;
+    static constexpr int SMEM_A_WS = 2 * CfgA::SMEM_A * 16 + NSTG_A_WS * CfgA::OP_DOUBLES * 8;
+    static constexpr int MINB_A_WS = pick_minb(SMEM_A_WS + kStaticA, 32 * (NAW + NBW), 96, 2, CfgA::NC * CfgA::TILES_PER_A);
+    static_assert(SMEM_C <= kMaxSmemAC && SMEM_A <= kMaxSmemAC && SMEM_A_WS <= kMaxSmemAC, "tile does not fit shared memory");
 };
 
 template <int TA, int TB, bool FREE, int CHUNK>

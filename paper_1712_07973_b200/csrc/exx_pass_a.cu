@@ -20,17 +20,19 @@ template <int TC, int TB, bool FREE>
 static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
     using T = TuneAC<TC, TB, FREE>;
     using C = typename T::CfgA;
-    constexpr int smem = T::SMEM_A;
-    static_assert(smem == C::SMEM_A * 16 + T::NSTG_A * C::OP_DOUBLES * 8, "pass A shared memory");
-    auto kern = pass_a_kernel<C, T::NT_A, T::NSTG_A, T::MINB_A>;
+    static_assert(T::SMEM_A == C::SMEM_A * 16 + T::NSTG_A * C::OP_DOUBLES * 8, "pass A shared memory");
+    constexpr bool ws = T::WS_A;
+    constexpr int smem = ws ? T::SMEM_A_WS : T::SMEM_A;
+    constexpr int nt = ws ? 32 * (T::NAW + T::NBW) : T::NT_A;
+    auto kern = ws ? pass_a_ws_kernel<C, T::NAW, T::NBW, T::NSTG_A_WS, T::MINB_A_WS> : pass_a_kernel<C, T::NT_A, T::NSTG_A, T::MINB_A>;
     static bool done = false;
     static int occ = 0;
-    if (info) { info->threads = T::NT_A; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
+    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
     if (!launch) return cudaSuccess;
-    cudaError_t e = prepare(kern, smem, T::NT_A, &done, &occ);
+    cudaError_t e = prepare(kern, smem, nt, &done, &occ);
     if (e != cudaSuccess) return e;
     if (info) info->ctas_per_sm = occ;
-    kern<<<args.na * C::TILES_PER_A, T::NT_A, smem, s>>>(args);
+    kern<<<args.na * C::TILES_PER_A, nt, smem, s>>>(args);
     return cudaGetLastError();
 }
 

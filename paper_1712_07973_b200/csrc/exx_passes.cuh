@@ -719,6 +719,96 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
 }
 
 
+// Pass A, warp-specialised variant (transform lengths >= 96).  NAW "line" warps run the co-density + c-axis FFT phases
+// A0, A1 of transform t+1 in one work buffer while NBW "column" warps run the first b-axis stage A2 of transform t out
+// of the other buffer and store it to W1, so the global-store-heavy phase overlaps the FP64-heavy ones and the CTA
+// needs no CTA-wide barrier: the buffers are handed over with mbarriers (sready: line -> column warps, sfree: back),
+// the line warps synchronise among themselves with a named barrier between A0 and A1.
+template <class C, int NAW, int NBW, int NSTG, int MINB>
+__global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_a_ws_kernel(const ArgsAC g) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* const S0 = reinterpret_cast<double2*>(smem_raw);            // two work buffers of SMEM_A
+    double* const OP = reinterpret_cast<double*>(S0 + 2 * C::SMEM_A);
+    __shared__ uint64_t full[NSTG], sready[2], sfree[2];
+    __shared__ double2 s_twc[C::TC], s_twb[C::TB];
+    constexpr int NT = 32 * (NAW + NBW), AT = 32 * NAW, BT = 32 * NBW;
+    const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
+        for (int b = 0; b < 2; ++b) { mbar_init(&sready[b], NAW); mbar_init(&sfree[b], NBW); }
+        mbar_fence_init();
+    }
+    for (int x = tid; x < C::TC; x += NT) s_twc[x] = g.twc[x];
+    for (int x = tid; x < C::TB; x += NT) s_twb[x] = g.twb[x];
+    __syncthreads();
+
+    if (tid < AT) {
+        // ------------------------------------------------------------------ line warps: A0, A1
+        constexpr int NI0 = ceil_div(C::ITEMS_LINE_Q, AT), NI1 = ceil_div(C::ITEMS_LINE_P, AT);
+        if (tid < 32)
+            for (int t = 0; t < NSTG && t < g.count; ++t)
+                issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+        LineQIdx q0[NI0];
+        double vj[NI0][C::PCN], vl[NI0][C::PCN];
+#pragma unroll
+        for (int m = 0; m < NI0; ++m) {
+            const int w = tid + m * AT;
+            q0[m] = lineq_index<C, false>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
+            const double* pj = g.psi + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
+            const double* pl = g.psi + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
+#pragma unroll
+            for (int n1 = 0; n1 < C::PCN; ++n1) { vj[m][n1] = ld_ro(pj + C::QC * n1); vl[m][n1] = ld_ro(pl + C::QC * n1); }
+        }
+        LinePIdx p1[NI1];
+#pragma unroll
+        for (int m = 0; m < NI1; ++m) p1[m] = linep_index<C, false>(tid + m * AT < C::ITEMS_LINE_P ? tid + m * AT : 0);
+
+        int flags_next = g.desc[0].flags;
+        for (int t = 0; t < g.count; ++t) {
+            const int s = t % NSTG, b = t & 1;
+            double2* const S = S0 + b * C::SMEM_A;
+            double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
+            const int flags = flags_next;
+            if (t + 1 < g.count) flags_next = g.desc[t + 1].flags;
+            if (t >= 2) mbar_wait(&sfree[b], ((t >> 1) - 1) & 1);      // the column warps have drained this buffer
+            mbar_wait(&full[s], (t / NSTG) & 1);
+#pragma unroll
+            for (int m = 0; m < NI0; ++m)
+                if (tid + m * AT < C::ITEMS_LINE_Q)
+                    a0_compute<C>(vj[m], vl[m], stage + q0[m].op, flags, S + q0[m].row, s_twc + q0[m].n2);
+            asm volatile("bar.sync 1, %0;" ::"n"(AT) : "memory");
+            if (tid < 32 && t + NSTG < g.count)                        // the stage has been consumed: refill it
+                issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+#pragma unroll
+            for (int m = 0; m < NI1; ++m)
+                if (tid + m * AT < C::ITEMS_LINE_P) a1_compute<C>(S + p1[m].seg);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sready[b]);
+        }
+    } else {
+        // ------------------------------------------------------------------ column warps: A2 -> W1
+        const int bt = tid - AT;
+        constexpr int NI2 = ceil_div(C::ITEMS_POS, BT);
+        ColIdx c2[NI2];
+#pragma unroll
+        for (int m = 0; m < NI2; ++m) c2[m] = col_index<C, false>(bt + m * BT < C::ITEMS_POS ? bt + m * BT : 0, a, b2base, g.na);
+        const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
+        for (int t = 0; t < g.count; ++t) {
+            const int b = t & 1;
+            double2* const S = S0 + b * C::SMEM_A;
+            double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
+            mbar_wait(&sready[b], (t >> 1) & 1);
+#pragma unroll
+            for (int m = 0; m < NI2; ++m)
+                if (bt + m * BT < C::ITEMS_POS) a2_compute<C>(S + c2[m].col, s_twb + c2[m].b2 * C::R1, w1t + c2[m].w1, qstride);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sfree[b]);
+        }
+    }
+}
+
 // Pass B.  Persistent CTAs over the (pch, q, t) blocks of the launch, t fastest (CTAs that run at the same time
 // share a K^ slice in L2).  The next block lands in a separate buffer by TMA bulk row copies while the current one is
 // transformed.  B0 / B4 map a thread to the rows (a, pin) it alone reads and writes, and the a-axis phases B1..B3 map
