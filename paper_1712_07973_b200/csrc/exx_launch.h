@@ -107,6 +107,11 @@ struct TuneAC {
     static constexpr int NSTG_A = 2;
     static constexpr int SMEM_A = smem_ac_bytes<TC, TB, FREE>(G_A, NSTG_A, false);
     static constexpr int MINB_A = pick_minb(SMEM_A + (TC + TB) * 16 + 64, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
+    // ---- pass C, warp-specialised: only where two tile buffers + two operand stages still let two CTAs share an SM
+    static constexpr bool WS_C = TC >= 96 && two_fit(2, 2);
+    static constexpr int NAW_C = 2;
+    static constexpr int NBW_C = imin(6, imax(1, (CfgC::ITEMS_LINE_Q + 31) / 32));
+    static constexpr int MINB_C_WS = pick_minb(SMEM_C + kStaticC, 32 * (NAW_C + NBW_C), 96, 2, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A, warp-specialised (lengths >= 96): line warps for A0/A1, column warps for A2, two work buffers
     static constexpr bool WS_A = TC >= 96;
     static constexpr int NAW = imin(6, imax(1, (imax(CfgA::ITEMS_LINE_Q, CfgA::ITEMS_LINE_P) + 31) / 32));

@@ -22,15 +22,18 @@ static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     using C = typename T::CfgC;
     constexpr int smem = T::SMEM_C;
     static_assert(smem == T::NBUF_C * C::SMEM_C * 16 + (T::NSTG_C * C::OP_DOUBLES + C::RES_DOUBLES) * 8, "pass C shared memory");
-    auto kern = pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C>;
+    static_assert(!T::WS_C || (T::NBUF_C == 2 && T::NSTG_C == 2), "warp-specialised pass C needs two buffers and two stages");
+    constexpr bool ws = T::WS_C;
+    constexpr int nt = ws ? 32 * (T::NAW_C + T::NBW_C) : T::NT_C;
+    auto kern = ws ? pass_c_ws_kernel<C, T::NAW_C, T::NBW_C, 2, T::MINB_C_WS> : pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C>;
     static bool done = false;
     static int occ = 0;
-    if (info) { info->threads = T::NT_C; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
+    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
     if (!launch) return cudaSuccess;
-    cudaError_t e = prepare(kern, smem, T::NT_C, &done, &occ);
+    cudaError_t e = prepare(kern, smem, nt, &done, &occ);
     if (e != cudaSuccess) return e;
     if (info) info->ctas_per_sm = occ;
-    kern<<<args.na * C::TILES_PER_A, T::NT_C, smem, s>>>(args);
+    kern<<<args.na * C::TILES_PER_A, nt, smem, s>>>(args);
     return cudaGetLastError();
 }
 

@@ -1195,6 +1195,154 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     if (tid < 32) bulk_wait_read_all();                    // shared memory must outlive the TMA reads
 }
 
+// Pass C, warp-specialised variant (used where two W1 tile buffers, two operand stages and two CTAs fit an SM).
+// NAW "column" warps gather the W1 tile of transform t+1 (16-byte cp.async) and run the inverse b-axis stage C0 in one
+// work buffer while NBW "line" warps run the inverse c-axis FFT C1, C2 and the Kernel-3 epilogue of transform t out of
+// the other, so the gather latency and the load-heavy phase overlap the FP64-heavy ones.  Buffers are handed over with
+// mbarriers (c0done: column -> line warps, sfree: back); the line warps synchronise among themselves with a named
+// barrier.  Arithmetic, accumulation order and the one-reduce-add-per-address rule are those of pass_c_kernel.
+template <class C, int NAW, int NBW, int NSTG, int MINB>
+__global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_c_ws_kernel(const ArgsAC g) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* const S0 = reinterpret_cast<double2*>(smem_raw);
+    double* const OP = reinterpret_cast<double*>(S0 + 2 * C::SMEM_C);
+    double* const RES = OP + NSTG * C::OP_DOUBLES;
+    __shared__ uint64_t full[NSTG], resbar, c0done[2], sfree[2];
+    __shared__ double red[2][NBW];
+    __shared__ double2 s_twct[C::TC], s_twb[C::TB];
+    constexpr int NT = 32 * (NAW + NBW), AT = 32 * NAW, BT = 32 * NBW;
+    const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
+        mbar_init(&resbar, 1);
+        for (int b = 0; b < 2; ++b) { mbar_init(&c0done[b], NAW); mbar_init(&sfree[b], NBW); }
+        mbar_fence_init();
+    }
+    for (int x = tid; x < C::TC; x += NT) s_twct[(x % C::QC) * C::PC + x / C::QC] = g.twc[x];
+    for (int x = tid; x < C::TB; x += NT) s_twb[x] = g.twb[x];
+    __syncthreads();
+
+    if (tid >= BT) {
+        // ------------------------------------------------------------------ column warps: W1 gather + C0
+        const int at = tid - BT;
+        constexpr int NI0 = ceil_div(C::ITEMS_POS, AT);
+        ColIdx c0[NI0];
+#pragma unroll
+        for (int m = 0; m < NI0; ++m) c0[m] = col_index<C, true>(at + m * AT < C::ITEMS_POS ? at + m * AT : 0, a, b2base, g.na);
+        const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
+        for (int t = 0; t < g.count; ++t) {
+            const int b = t & 1;
+            double2* const S = S0 + b * C::SMEM_C;
+            const double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
+            if (t >= 2) mbar_wait(&sfree[b], ((t >> 1) - 1) & 1);      // the line warps have drained this buffer
+#pragma unroll
+            for (int m = 0; m < NI0; ++m)
+                if (at + m * AT < C::ITEMS_POS) {
+#pragma unroll
+                    for (int q = 0; q < C::R1; ++q) cp_async16(S + c0[m].col + q * C::ROW, w1t + c0[m].w1 + q * qstride);
+                }
+            cp_async_commit();
+            cp_async_wait<0>();
+#pragma unroll
+            for (int m = 0; m < NI0; ++m)
+                if (at + m * AT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, s_twb + c0[m].b2 * C::R1);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&c0done[b]);
+        }
+    } else {
+        // ------------------------------------------------------------------ line warps: C1, C2, epilogue
+        constexpr int NI1 = ceil_div(C::ITEMS_LINE_P, BT), NI2 = ceil_div(C::ITEMS_LINE_Q, BT);
+        if (tid < 32) {
+            if (tid == 0) mbar_arrive_expect_tx(&resbar, 2 * C::LINES * C::LINE_BYTES);
+            __syncwarp();
+            issue_line_loads<C>(g, g.j, RES, &resbar, a, b2base, tid);
+            issue_line_loads<C>(g, g.l >= 0 ? g.l : g.j, RES + C::LINES * C::LS, &resbar, a, b2base, tid);
+            for (int t = 0; t < NSTG && t < g.count; ++t)
+                issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+        }
+        LinePIdx p1[NI1];
+#pragma unroll
+        for (int m = 0; m < NI1; ++m) p1[m] = linep_index<C, true>(tid + m * BT < C::ITEMS_LINE_P ? tid + m * BT : 0);
+        LineQIdx q2[NI2];
+        double accj[NI2][C::PCN], accl[NI2][C::PCN];
+#pragma unroll
+        for (int m = 0; m < NI2; ++m) {
+            const int w = tid + m * BT;
+            q2[m] = lineq_index<C, true>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
+#pragma unroll
+            for (int n1 = 0; n1 < C::PCN; ++n1) { accj[m][n1] = 0.0; accl[m][n1] = 0.0; }
+        }
+        XformDesc d_next = g.desc[0];
+        for (int t = 0; t < g.count; ++t) {
+            const int b = t & 1, s = t % NSTG;
+            double2* const S = S0 + b * C::SMEM_C;
+            double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
+            const XformDesc d = d_next;
+            if (t + 1 < g.count) d_next = g.desc[t + 1];
+            mbar_wait(&c0done[b], (t >> 1) & 1);
+#pragma unroll
+            for (int m = 0; m < NI1; ++m)
+                if (tid + m * BT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, s_twct + p1[m].k1, C::PC, p1[m].k1);
+            asm volatile("bar.sync 1, %0;" ::"n"(BT) : "memory");
+            if (t == 0) mbar_wait(&resbar, 0);
+            mbar_wait(&full[s], (t / NSTG) & 1);
+            double e1 = 0.0, e2 = 0.0;
+#pragma unroll
+            for (int m = 0; m < NI2; ++m)
+                if (tid + m * BT < C::ITEMS_LINE_Q)
+                    c2_compute<C>(S + q2[m].row, d, g.l, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                                  accj[m], accl[m], e1, e2);
+            fence_proxy_async();
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                e1 += __shfl_xor_sync(0xffffffffu, e1, o);
+                e2 += __shfl_xor_sync(0xffffffffu, e2, o);
+            }
+            if (lane == 0) {
+                red[0][tid >> 5] = e1; red[1][tid >> 5] = e2;
+                mbar_arrive(&sfree[b]);                                // this warp no longer reads the work buffer
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(BT) : "memory");      // operand stage and red[] complete
+            if (tid == 0) {
+                double s1 = 0.0, s2 = 0.0;
+#pragma unroll
+                for (int k = 0; k < NBW; ++k) { s1 += red[0][k]; s2 += red[1][k]; }
+                double* ep = g.epart + (static_cast<size_t>(t) * gridDim.x + tile) * 2;
+                ep[0] = s1; ep[1] = s2;
+            }
+            if (tid < 32) {
+                if (d.flags != 0 && d.i != g.j && d.i != g.l) {
+                    double* ki = g.kpsi + static_cast<size_t>(d.i) * g.m_points;
+                    for (int l = tid; l < C::LINES; l += 32)
+                        bulk_red_add_f64(ki + line_offset<C>(l, a, b2base), stage + l * C::LS, C::LINE_BYTES);
+                }
+                bulk_commit();
+                if (t + NSTG < g.count) {
+                    bulk_wait_read_all();
+                    __syncwarp();
+                    issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+                }
+            }
+            // red[] is rewritten only after the next named barrier pair, the stage only after its mbarrier: no hazard
+        }
+#pragma unroll
+        for (int m = 0; m < NI2; ++m)
+            if (tid + m * BT < C::ITEMS_LINE_Q) {
+                double* kj = g.kpsi + static_cast<size_t>(g.j) * g.m_points + q2[m].gofs;
+#pragma unroll
+                for (int n1 = 0; n1 < C::PCN; ++n1) kj[C::QC * n1] -= accj[m][n1];
+                if (g.l >= 0) {
+                    double* kl = g.kpsi + static_cast<size_t>(g.l) * g.m_points + q2[m].gofs;
+#pragma unroll
+                    for (int n1 = 0; n1 < C::PCN; ++n1) kl[C::QC * n1] -= accl[m][n1];
+                }
+            }
+        if (tid < 32) bulk_wait_read_all();
+    }
+}
+
 #endif  // __CUDACC__
 
 }  // namespace exx
