@@ -113,6 +113,28 @@ def test_apply_is_repeatable_and_overwrites():
     plan.destroy()
 
 
+@pytest.mark.parametrize("base,dims", [("C1", (96, 96, 96)), ("C2", (48, 48, 48))])
+def test_warp_specialised_kernels_repeat_bitwise(base, dims):
+    """Transform length 96: all three passes run their warp-specialised kernels (mbarrier hand-over between warp
+    roles).  A race there shows up as run-to-run differences: five applies, several batch cuts, bit-identical."""
+    w = make_workload(small_spec(base, dims=dims, n_orb=7, number=91))
+    spec = w["spec"]
+    psi = w["psi"].cuda()
+    plan = exx.ExxPlan(spec.dims, spec.spacing, spec.bc, w["kernel"], max_orbitals=spec.n_orb)
+    ref_k, ref_ex = plan.apply(psi, w["occ"])
+    ref_k = ref_k.clone()
+    for batch in (0, 1, 2, 3, 5):
+        plan.set_batch(batch)
+        k, ex = plan.apply(psi, w["occ"])
+        if batch == 0:
+            assert torch.equal(k, ref_k) and ex == ref_ex
+        else:                                               # other batch cuts change the accumulation order of K psi_j only
+            assert float((k - ref_k).abs().max()) <= 1e-13 * float(ref_k.abs().max())
+            k2, ex2 = plan.apply(psi, w["occ"])
+            assert torch.equal(k, k2) and ex == ex2
+    plan.destroy()
+
+
 def test_pointer_and_argument_errors():
     w = make_workload(small_spec("C1", dims=(16, 16, 16), n_orb=2, number=79))
     plan = exx.ExxPlan((16, 16, 16), w["spec"].spacing, "periodic", None, max_orbitals=2)
