@@ -81,6 +81,17 @@ constexpr int pick_minb(int smem, int nt, int reg_floor, int cap, int tiles) {  
     return best;
 }
 
+// warps (<= cap) for `items` equal work items: the count that wastes the fewest lane-rounds, ties -> more warps
+constexpr int pick_line_warps(int items, int cap) {
+    int best = 1, best_waste = 1 << 30;
+    for (int w = 1; w <= cap; ++w) {
+        const int rounds = (items + 32 * w - 1) / (32 * w);
+        const int waste = rounds * 32 * w - items;
+        if (waste <= best_waste) { best_waste = waste; best = w; }
+    }
+    return best;
+}
+
 template <int TC, int TB, bool FREE>
 struct TuneAC {
     static constexpr int CHUNK = chunk_for(TC, TB, FREE);
@@ -110,11 +121,11 @@ struct TuneAC {
     // ---- pass C, warp-specialised: only where two tile buffers + two operand stages still let two CTAs share an SM
     static constexpr bool WS_C = TC >= 96 && two_fit(2, 2);
     static constexpr int NAW_C = 2;
-    static constexpr int NBW_C = imin(6, imax(1, (CfgC::ITEMS_LINE_Q + 31) / 32));
+    static constexpr int NBW_C = pick_line_warps(CfgC::ITEMS_LINE_Q, 6);
     static constexpr int MINB_C_WS = pick_minb(SMEM_C + kStaticC, 32 * (NAW_C + NBW_C), 96, 2, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A, warp-specialised (lengths >= 96): line warps for A0/A1, column warps for A2, two work buffers
     static constexpr bool WS_A = TC >= 96;
-    static constexpr int NAW = imin(6, imax(1, (imax(CfgA::ITEMS_LINE_Q, CfgA::ITEMS_LINE_P) + 31) / 32));
+    static constexpr int NAW = pick_line_warps(imax(CfgA::ITEMS_LINE_Q, CfgA::ITEMS_LINE_P), 6);
     static constexpr int NBW = imax(2, 8 - NAW);
     static constexpr int kStaticA = (TC + TB) * 16 + 128;
     static constexpr int NSTG_A_WS =                       // one operand stage if that is what lets two CTAs share an SM
