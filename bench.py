@@ -273,8 +273,7 @@ def main():
     dom_ms_per_launch = pass_ms[dom] / max(1, pass_n[dom])
     dom_bytes_per_launch = per_x[dom_name] * n_xforms / max(1, pass_n[dom])
     achieved = dom_bytes_per_launch / (dom_ms_per_launch * 1e-3) / 1e9
-    kernel_name = {"A": "pass_a_kernel", "C": "pass_c_kernel",
-                   "B": "pass_b_ws_kernel" if max(plan.transform_dims()) >= 96 else "pass_b_kernel"}[dom_name]
+    kernel_name = plan.kernel_name(dom)
     roofline = {"bound": "hbm", "kernel": kernel_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": _ncu_traffic(args.config, dom_name, n_xforms / max(1, pass_n[dom])),
                 "peak_source": peak_src,

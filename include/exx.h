@@ -116,6 +116,10 @@ exx_status exx_schedule_list(int n_orb, const double *occ_host, int max_batch, i
 exx_status exx_plan_transform_dims(const exx_plan *plan, int tdims[3]);
 size_t     exx_plan_workspace_bytes(const exx_plan *plan);
 
+/* Name of the kernel this plan's geometry dispatches to for pass 0 (A), 1 (B) or 2 (C); "" for anything else.  The
+ * string is static, owned by the library. */
+const char *exx_plan_kernel_name(const exx_plan *plan, int pass);
+
 /* Number of kernel launches the library has enqueued for this plan since creation (for bench "gpu_launches"). */
 long long  exx_plan_launch_count(const exx_plan *plan);
 

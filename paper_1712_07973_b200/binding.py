@@ -22,7 +22,7 @@ _STATUS = ["EXX_OK", "EXX_ERR_INVALID_ARG", "EXX_ERR_UNSUPPORTED_SIZE", "EXX_ERR
 
 EXPORTS = [
     "exx_plan_create", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_get_pair_energies",
-    "exx_schedule_pairs", "exx_schedule_list", "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count",
+    "exx_schedule_pairs", "exx_schedule_list", "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_kernel_name",
     "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version",
 ]
 
@@ -66,6 +66,8 @@ def load_library():
     lib.exx_plan_transform_dims.restype = C.c_int
     lib.exx_plan_workspace_bytes.argtypes = [C.c_void_p]
     lib.exx_plan_workspace_bytes.restype = C.c_size_t
+    lib.exx_plan_kernel_name.argtypes = [C.c_void_p, C.c_int]
+    lib.exx_plan_kernel_name.restype = C.c_char_p
     lib.exx_plan_launch_count.argtypes = [C.c_void_p]
     lib.exx_plan_launch_count.restype = C.c_longlong
     lib.exx_plan_set_batch.argtypes = [C.c_void_p, C.c_int]
@@ -158,6 +160,10 @@ class ExxPlan:
 
     def launch_count(self) -> int:
         return int(load_library().exx_plan_launch_count(self._h))
+
+    def kernel_name(self, pass_index: int) -> str:
+        """Kernel this plan dispatches to for pass 0 (A), 1 (B), 2 (C)."""
+        return load_library().exx_plan_kernel_name(self._h, int(pass_index)).decode()
 
     def set_batch(self, n: int):
         self._check(load_library().exx_plan_set_batch(self._h, int(n)))

@@ -650,6 +650,12 @@ size_t exx_plan_workspace_bytes(const exx_plan* p) { return p ? p->ws_bytes + p-
 
 long long exx_plan_launch_count(const exx_plan* p) { return p ? p->launches : 0; }
 
+const char* exx_plan_kernel_name(const exx_plan* p, int pass) {
+    if (!p) return "";
+    const KernelInfo& k = pass == 0 ? p->info_a : pass == 1 ? p->info_b : p->info_c;
+    return (pass >= 0 && pass <= 2 && k.name) ? k.name : "";
+}
+
 exx_status exx_plan_set_profiling(exx_plan* p, int enable) {
     if (!p) return EXX_ERR_INVALID_ARG;
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));

@@ -19,6 +19,7 @@ struct KernelInfo {     // what a launcher reports about the instantiation it di
     int smem_bytes;
     int tiles;           // pass A / C: CTAs per launch (na * R2 / G);  pass B: blocks per transform (R1 * TC / CHUNK)
     int ctas_per_sm;     // occupancy the launcher sized its grid for (pass B: persistent grid = SMs * this)
+    const char* name;    // kernel the launcher dispatches to for this geometry
 };
 
 // Transform lengths the FFT covers.

@@ -27,7 +27,7 @@ static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     auto kern = ws ? pass_a_ws_kernel<C, T::NAW, T::NBW, T::NSTG_A_WS, T::MINB_A_WS> : pass_a_kernel<C, T::NT_A, T::NSTG_A, T::MINB_A>;
     static bool done = false;
     static int occ = 0;
-    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
+    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; info->name = ws ? "pass_a_ws_kernel" : "pass_a_kernel"; }
     if (!launch) return cudaSuccess;
     cudaError_t e = prepare(kern, smem, nt, &done, &occ);
     if (e != cudaSuccess) return e;

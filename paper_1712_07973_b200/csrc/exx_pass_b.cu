@@ -39,7 +39,7 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
                   : T::WSF ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB, true> : pass_b_kernel<C, T::NT, T::MINB>;
         static bool done = false;
         static int occ = 0;
-        if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; }
+        if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; info->name = (T::WS || T::WSF) ? "pass_b_ws_kernel" : "pass_b_kernel"; }
         if (!launch) return cudaSuccess;
         cudaError_t e = prepare(kern, T::SMEM, T::NT, &done, &occ);
         if (e != cudaSuccess) return e;

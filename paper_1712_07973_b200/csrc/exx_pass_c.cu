@@ -28,7 +28,7 @@ static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     auto kern = ws ? pass_c_ws_kernel<C, T::NAW_C, T::NBW_C, 2, T::MINB_C_WS> : pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C>;
     static bool done = false;
     static int occ = 0;
-    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; }
+    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; info->name = ws ? "pass_c_ws_kernel" : "pass_c_kernel"; }
     if (!launch) return cudaSuccess;
     cudaError_t e = prepare(kern, smem, nt, &done, &occ);
     if (e != cudaSuccess) return e;
