@@ -121,7 +121,7 @@ struct TuneAC {
     static constexpr int MINB_A = pick_minb(SMEM_A + (TC + TB) * 16 + 64, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
     // ---- pass C, warp-specialised: only where two tile buffers + two operand stages still let two CTAs share an SM
     static constexpr bool WS_C = TC >= 96 && two_fit(2, 2);
-    static constexpr int NAW_C = 2;
+    static constexpr int NAW_C = 1;                        // one gather + C0 warp keeps up with six line warps (measured)
     static constexpr int NBW_C = pick_line_warps(CfgC::ITEMS_LINE_Q, 6);
     static constexpr int MINB_C_WS = pick_minb(SMEM_C + kStaticC, 32 * (NAW_C + NBW_C), 96, 2, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A, warp-specialised (lengths >= 96): line warps for A0/A1, column warps for A2, two work buffers
@@ -144,7 +144,7 @@ struct TuneB {
     // to feed both kinds of warps: WS with two full work buffers, else (free BC) WSF with NA-row buffers and per-warp
     // expansion scratch; else work + landing buffer with CTA barriers
     static constexpr int NY = Cfg::NGRP <= 12 ? Cfg::NGRP : Cfg::NGRP / 2;       // column warps
-    static constexpr int NX = 4;                                                // row warps
+    static constexpr int NX = 4;                                                // row warps (2, 3, 5, 6 measured slower)
     static constexpr bool kBig = Cfg::NGRP >= 6 && (Cfg::NGRP <= 12 || Cfg::NGRP % 2 == 0);
     static constexpr int SMEM_WS = (2 * Cfg::WORK_ELEMS + 2 * TA) * 16;
     static constexpr int SMEM_WSF = (2 * Cfg::P_ELEMS + NY * Cfg::E_ELEMS + 2 * TA) * 16;
