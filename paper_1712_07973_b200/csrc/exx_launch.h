@@ -121,7 +121,9 @@ struct TuneAC {
     static constexpr int MINB_A = pick_minb(SMEM_A + (TC + TB) * 16 + 64, NT_A, 96, 4, CfgA::NC * CfgA::TILES_PER_A);
     // ---- pass C, warp-specialised: only where two tile buffers + two operand stages still let two CTAs share an SM
     static constexpr bool WS_C = TC >= 96 && two_fit(2, 2);
-    static constexpr int NAW_C = 1;                        // one gather + C0 warp keeps up with six line warps (measured)
+    // gather + C0 warps: one keeps up with six line warps for periodic grids (measured); the pruned 2n-point stage of
+    // free BC carries a larger share of the work
+    static constexpr int NAW_C = FREE ? 2 : 1;
     static constexpr int NBW_C = pick_line_warps(CfgC::ITEMS_LINE_Q, 6);
     static constexpr int MINB_C_WS = pick_minb(SMEM_C + kStaticC, 32 * (NAW_C + NBW_C), 96, 2, CfgC::NC * CfgC::TILES_PER_A);
     // ---- pass A, warp-specialised (lengths >= 96): line warps for A0/A1, column warps for A2, two work buffers
