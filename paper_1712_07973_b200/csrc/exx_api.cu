@@ -157,7 +157,6 @@ struct exx_plan {
     int max_batch;
     cudaStream_t stream;
     double2* tw[3];
-    double2* roots[3];
     double2* twb;           // [b2*R1 + q] = W_TB^{b2 q}
     double* ks;             // [TB/2+1][TC][TA/2+1], c index in scrambled order (see permute_kernel_axes)
     double2* w1;
@@ -238,8 +237,6 @@ void host_tables(int T, std::vector<double2>& tw, std::vector<double2>& roots) {
 }
 
 void split_of(int T, int* P, int* Q) {
-    std::vector<double2> a, b;
-    (void)a; (void)b;
     switch (T) {
         case 16: *P = Split<16>::P; *Q = Split<16>::Q; break;
         case 32: *P = Split<32>::P; *Q = Split<32>::Q; break;
@@ -554,12 +551,11 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
         std::vector<double2> tw, roots;
         host_tables(p->t[ax], tw, roots);
         const size_t bytes = sizeof(double2) * p->t[ax];
-        if (cudaMalloc(&p->tw[ax], bytes) != cudaSuccess || cudaMalloc(&p->roots[ax], bytes) != cudaSuccess) {
+        if (cudaMalloc(&p->tw[ax], bytes) != cudaSuccess) {
             cudaGetLastError();
             return bail(fail(p, EXX_ERR_ALLOC, "cudaMalloc(twiddles) failed"));
         }
-        if (cudaMemcpy(p->tw[ax], tw.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(p->roots[ax], roots.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+        if (cudaMemcpy(p->tw[ax], tw.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
             cudaGetLastError();
             return bail(fail(p, EXX_ERR_CUDA, "twiddle upload failed"));
         }
@@ -616,7 +612,6 @@ exx_status exx_plan_destroy(exx_plan* p) {
     if (p->stream || p->w1) cudaStreamSynchronize(p->stream);
     for (int ax = 0; ax < 3; ++ax) {
         if (p->tw[ax]) cudaFree(p->tw[ax]);
-        if (p->roots[ax]) cudaFree(p->roots[ax]);
     }
     if (p->ks) cudaFree(p->ks);
     if (p->twb) cudaFree(p->twb);
