@@ -135,6 +135,18 @@ def test_warp_specialised_kernels_repeat_bitwise(base, dims):
     plan.destroy()
 
 
+@pytest.mark.parametrize("base,dims", [("C1", (96, 96, 96)), ("C2", (48, 48, 48))])
+def test_warp_specialised_kernels_edge_schedule(base, dims):
+    """Odd N, zero occupations (absent real / imaginary slots, skipped transforms) and one- and three-transform batches
+    through the warp-specialised kernels, element by element against the oracle's N^2 definition."""
+    w = make_workload(small_spec(base, dims=dims, n_orb=7, number=92))
+    occ = [0.0, 1.2, 0.0, 2.0, 0.0, 0.0, 0.7]
+    ex_a = _check_full(w, occ=occ, symmetric=False)
+    ex_b = _check_full(w, occ=occ, symmetric=False, batch=1)
+    ex_c = _check_full(w, occ=occ, symmetric=False, batch=3)
+    assert abs(ex_a - ex_b) <= 1e-13 * abs(ex_a) and abs(ex_a - ex_c) <= 1e-13 * abs(ex_a)
+
+
 def test_pointer_and_argument_errors():
     w = make_workload(small_spec("C1", dims=(16, 16, 16), n_orb=2, number=79))
     plan = exx.ExxPlan((16, 16, 16), w["spec"].spacing, "periodic", None, max_orbitals=2)
