@@ -143,6 +143,67 @@ def cpu_baseline(spec, w, seconds_target=15.0):
                       f"{total_time:.1f} s wall"}
 
 
+def cufft_comparison(spec, psi, occ, kernel_table, plan_pair_energies, seconds_target=2.0):
+    """GPU comparison baseline ("the cuFFT path ... same inputs, same metric"; reported, never the
+    product): the textbook pipeline on library calls -- co-densities as a torch product, torch.fft.rfftn / irfftn
+    (cuFFT D2Z / Z2D, zero-padded to 2n for free BC), pointwise multiply by K^, pointwise epilogue -- timed on a bounded
+    sample of rows i (all j >= i of a row, batched).  Returns pair-solves/s and a sanity check against the library."""
+    import torch
+    n = spec.dims
+    free = spec.bc == "free"
+    t = tuple(2 * d for d in n) if free else tuple(n)
+    dev = psi.device
+    if free:
+        g = torch.as_tensor(kernel_table, dtype=torch.float64, device=dev)
+        ext = torch.zeros(t, dtype=torch.float64, device=dev)
+        idx = [torch.minimum(torch.arange(tt, device=dev), tt - torch.arange(tt, device=dev)) for tt in t]
+        mask = [(i != tt // 2) for i, tt in zip(idx, t)]
+        ext = g[idx[0].clamp(max=n[0] - 1)][:, idx[1].clamp(max=n[1] - 1)][:, :, idx[2].clamp(max=n[2] - 1)]
+        ext = ext * (mask[0][:, None, None] & mask[1][None, :, None] & mask[2][None, None, :])
+        khat = torch.fft.rfftn(ext).real * spec.dV
+    else:
+        freq = [2.0 * np.pi * torch.fft.fftfreq(tt, d=h, device=dev, dtype=torch.float64) for tt, h in zip(t, spec.spacing)]
+        g2 = freq[0][:, None, None] ** 2 + freq[1][None, :, None] ** 2 + (freq[2][None, None, : t[2] // 2 + 1]) ** 2
+        khat = torch.where(g2 > 0, 4.0 * np.pi / g2.clamp(min=1e-300), torch.zeros_like(g2))
+    n_orb = psi.shape[0]
+    kpsi = torch.zeros_like(psi)
+    bmax = max(1, int(2e9 // (8 * t[0] * t[1] * t[2])))              # about 2 GB of padded real co-densities per batch
+    sl = tuple(slice(0, d) for d in n)
+
+    def row(i):
+        e_row = torch.zeros(n_orb, dtype=torch.float64, device=dev)
+        for j0 in range(i, n_orb, bmax):
+            js = slice(j0, min(n_orb, j0 + bmax))
+            rho = psi[i][None] * psi[js]
+            v = torch.fft.irfftn(torch.fft.rfftn(rho, s=t, dim=(1, 2, 3)) * khat, s=t, dim=(1, 2, 3))[(slice(None),) + sl]
+            kpsi[i] -= torch.einsum("j,jabc->abc", torch.as_tensor(occ[js], device=dev), v * psi[js])
+            off = torch.as_tensor(occ[i] * (np.arange(js.start, js.stop) != i), device=dev)
+            kpsi[js] -= off[:, None, None, None] * v * psi[i][None]
+            e_row[js] = spec.dV * (rho * v).sum(dim=(1, 2, 3))
+        return e_row
+
+    rows = [0]
+    e0 = row(0)                                                     # warm-up (cuFFT plans) and the sanity row
+    torch.cuda.synchronize()
+    ref = torch.as_tensor(plan_pair_energies[0], device=dev)
+    err = float((e0 - ref).abs().max() / ref.abs().max())
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pairs, ms = 0, 0.0
+    rng = np.random.default_rng(7)
+    while ms < seconds_target * 1e3 and len(rows) < 64:
+        i = int(rng.integers(0, n_orb))
+        ev0.record()
+        row(i)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms += ev0.elapsed_time(ev1)
+        pairs += n_orb - i
+        rows.append(i)
+    return {"value": pairs / (ms * 1e-3), "unit": UNIT, "kind": "torch.fft (cuFFT D2Z/Z2D) + pointwise torch ops, one real co-density per transform",
+            "sample": f"{pairs} pair solves ({len(rows) - 1} seeded rows i, all j >= i), {ms * 1e-3:.2f} s device time",
+            "max_rel_err_pair_energies_row0_vs_library": err}
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle on the same config/metric; each step a bounded sample of the workload."""
     if rank != 0:
@@ -190,6 +251,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="max packed transforms per batch (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--compare-cufft", action="store_true", help="also time a torch.fft (cuFFT) pipeline on a sample, as a comparison")
     args = ap.parse_args()
     if args.steps is None:
         args.steps = {"C1": 20, "C2": 10, "C3": 5, "C4": 3, "C5": 1}[args.config]
@@ -316,6 +378,10 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(spec, w)
+    cufft = None
+    if rank == 0 and world == 1 and args.compare_cufft and psi.numel() * 8 <= 24e9:
+        plan.apply_async(psi, occ, kpsi, ex_dev)
+        cufft = cufft_comparison(spec, psi, occ, w["kernel"], plan.pair_energies(spec.n_orb))
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -326,7 +392,7 @@ def main():
                            "parallelism": "replicas" if world > 1 else "single GPU",
                            "workspace_bytes": plan.workspace_bytes()},
                 "apply_seconds": step_ms * 1e-3, "E_x": ex_value, "clocks": clocks, "gpu_launches": int(launches),
-                "e2e": e2e, "roofline": roofline, "roofline_path": roofline_path, "cpu_baseline": cpu}
+                "e2e": e2e, "roofline": roofline, "roofline_path": roofline_path, "cpu_baseline": cpu, "cufft_comparison": cufft}
         print(json.dumps(line))
     plan.destroy()
     if distributed:
