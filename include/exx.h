@@ -23,8 +23,10 @@
  * periodic kernel 4 pi/|G|^2 with the G=0 term set to 0; free kernel = host table, Hockney padding to 2n.
  *
  * Memory order: psi[i][a][b][c], C order, c fastest: index = ((i*n1 + a)*n2 + b)*n3 + c.
- * Threading: a plan is not re-entrant; distinct plans are independent.  All device work is enqueued on the
- * plan's stream.  No entry point throws, aborts or exits; errors are status codes plus exx_last_error text.
+ * Threading: a plan is not re-entrant; distinct plans (also on different devices) are independent.  All device work
+ * is enqueued on the plan's stream.  No entry point throws, aborts or exits; errors are status codes plus
+ * exx_last_error text.  The apply calls perform no host or device allocation (the one exception: exx_apply_host grows
+ * its device staging buffers when n_orb exceeds every earlier call's).
  */
 #ifndef EXX_B200_H
 #define EXX_B200_H
@@ -56,9 +58,14 @@ typedef enum { EXX_BC_PERIODIC = 0, EXX_BC_FREE = 1 } exx_bc;
  *               {16, 32, 64, 96, 128, 192, 256} (radix-2/3 only), else EXX_ERR_UNSUPPORTED_SIZE.
  *   spacing     HOST, h1,h2,h3 in bohr (> 0).
  *   bc          EXX_BC_PERIODIC or EXX_BC_FREE.
- *   kernel_host HOST.  PERIODIC: NULL => analytic 4 pi/|G|^2, G = 0 -> 0.  (A non-NULL pointer is rejected.)
+ *   kernel_host HOST.  PERIODIC: NULL => analytic 4 pi/|G|^2, G = 0 -> 0.  Non-NULL => Fourier-space filter table
+ *               K^[s1][s2][s3] of (n1/2+1)*(n2/2+1)*(n3/2+1) doubles on the symmetric index range (frequency index
+ *               m_a = +-s_a, G_a = 2 pi m_a / (n_a h_a); K^ is taken even in every index), WITHOUT the 1/(n1 n2 n3)
+ *               of the inverse transform -- e.g. the screened kernel of HSE06-type hybrids, "only the filter F of
+ *               kernel 2 would be different".
  *               FREE: table g[a][b][c] of n1*n2*n3 doubles = Green's function at displacement
- *               (a h1, b h2, c h3), units 1/bohr; copied during the call, caller may free it afterwards.
+ *               (a h1, b h2, c h3), units 1/bohr (an interpolating-scaling-function table can be passed as is).
+ *               Either table is copied during the call; the caller may free it afterwards.
  *   max_orbitals  upper bound for n_orb of later exx_apply calls (sizes the pair-energy buffers).
  *   cuda_stream cudaStream_t as void* (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream.
  * On success *plan receives a handle that the caller must release with exx_plan_destroy.
@@ -89,10 +96,71 @@ exx_status exx_apply_host(exx_plan *plan, int n_orb, const double *psi_host, con
                           double *kpsi_host, double *ex_host);
 
 /*
- * exx_get_pair_energies -- e_ij = dV sum_r rho_ij(r) V_ij(r) of the most recent apply, HOST [n_orb*n_orb],
- * symmetric (Eq. 5 integrand).  Pairs skipped for zero occupations read 0.  Synchronises.
+ * exx_plan_release_staging -- frees the device staging buffers exx_apply_host keeps between calls (2 * n_orb * n1*n2*n3
+ * doubles: the algorithm needs every orbital and every K psi row resident; they count in exx_plan_workspace_bytes).
  */
-exx_status exx_get_pair_energies(exx_plan *plan, double *e_host);
+exx_status exx_plan_release_staging(exx_plan *plan);
+
+/*
+ * exx_get_pair_energies -- e_ij = dV sum_r rho_ij(r) V_ij(r) of the most recent exx_apply / _async / _host / _pairs,
+ * HOST [n_orb*n_orb], symmetric (Eq. 5 integrand).  n_orb must equal that apply's orbital count
+ * (EXX_ERR_INVALID_ARG otherwise: the buffer size is the caller's statement, never guessed).  Pairs skipped for zero
+ * occupations or by a pair mask read 0.  Synchronises.
+ */
+exx_status exx_get_pair_energies(exx_plan *plan, int n_orb, double *e_host);
+
+/*
+ * exx_apply_pairs -- exx_apply restricted to a caller-supplied list of pairs: localised orbitals, for which "the
+ * matrix K^{alpha beta} is sparse" (Eq. 6-7) because co-densities of non-overlapping orbitals vanish.
+ *   pair_mask_host  HOST, [n_orb*n_orb] bytes, symmetric; pair (a,b) is solved iff mask[a*n_orb+b] != 0 (and not both
+ *                   occupations are zero).  Excluded pairs contribute nothing to K psi, E_x and read 0 in e_ij.
+ * Other arguments as exx_apply.  EXX_ERR_INVALID_ARG for an asymmetric mask.
+ */
+exx_status exx_apply_pairs(exx_plan *plan, int n_orb, const double *psi_dev, const double *occ_host,
+                           const unsigned char *pair_mask_host, double *kpsi_dev, double *ex_host);
+
+/*
+ * exx_apply_to -- the exchange operator built from the occupied set applied to ANOTHER set of orbitals (unoccupied /
+ * virtual states, a trial subspace; the second spin channel is a second call with that channel's occupied set --
+ * PAPER.md:210, Table 3 caption :244; Eq. 3 :67-69 with phi_t in place of psi_i):
+ *      K phi_t (r) = - sum_j f_j  V[phi_t psi_j](r)  psi_j(r),      j over the n_occ occupied orbitals.
+ *   psi_dev   DEVICE [n_occ][n1][n2][n3], occ_host HOST [n_occ] (orbitals with f_j = 0 are skipped);
+ *   phi_dev   DEVICE [n_tgt][n1][n2][n3];  kphi_dev DEVICE, same shape as phi, OVERWRITTEN.
+ * n_occ, n_tgt <= max_orbitals; all arrays 16-byte aligned; kphi must not overlap psi or phi (phi may be psi).  No
+ * energy is produced.  Synchronises the plan's stream before returning.
+ */
+exx_status exx_apply_to(exx_plan *plan, int n_occ, const double *psi_dev, const double *occ_host, int n_tgt,
+                        const double *phi_dev, double *kphi_dev);
+
+/*
+ * exx_apply_block -- all pairs BETWEEN two disjoint orbital blocks, the unit of work of the paper's round-robin
+ * distribution (Fig. 1: each process "calculates the co-densities between its own orbitals and the
+ * received ones"; the potential serves both orbitals of a pair):  for every j in the resident block, i in the streamed one
+ *      kpsi_res[j] -= f_i V_ji psi_i ,   kpsi_str[i] -= f_j V_ji psi_j ,   e_ji = dV sum_r rho_ji V_ji ,
+ *      *ex_host = - sum_{j,i} f_j f_i e_ji     (the block's whole contribution to E_x: Eq. 5 counts (j,i) and (i,j)).
+ *   flags  EXX_BLOCK_ACCUMULATE_RESIDENT / _STREAMED: add to the existing content of kpsi_res / kpsi_str instead of
+ *          overwriting it (partial results of successive round-robin steps).
+ * The two blocks must not share memory (use exx_apply for a block with itself); sub-ranges of one array are fine.
+ * exx_get_block_energies returns e_ji of the most recent call, HOST [n_res*n_str].  Synchronises.
+ */
+enum { EXX_BLOCK_ACCUMULATE_RESIDENT = 1, EXX_BLOCK_ACCUMULATE_STREAMED = 2 };
+exx_status exx_apply_block(exx_plan *plan, int n_res, const double *psi_res_dev, const double *occ_res_host,
+                           double *kpsi_res_dev, int n_str, const double *psi_str_dev, const double *occ_str_host,
+                           double *kpsi_str_dev, int flags, double *ex_host);
+exx_status exx_get_block_energies(exx_plan *plan, int n_res, int n_str, double *e_host);
+
+/*
+ * exx_round_robin_step -- HOST-only schedule of the paper's round-robin exchange (Fig. 1; "[P/2]+1"
+ * steps, reading A16: floor).  At step s = 0..floor(P/2) rank p sends its own orbital block to rank
+ * *send_to = (p+s) mod P, receives the block of *recv_from = (p-s) mod P and computes, *what =
+ *   0  the diagonal block (s = 0: exx_apply on its own orbitals; nothing is exchanged),
+ *   1  the full block own (resident) x received (streamed) with exx_apply_block,
+ *   2  even P, last step, p < recv_from: resident = FIRST half of the own block (rows [0, ceil(n_own/2))), streamed = the whole received block,
+ *   3  even P, last step, p > recv_from: resident = the whole own block, streamed = SECOND half of the received block
+ *      (rows [ceil(n_recv/2), n_recv)) -- together the two ranks cover that block pair exactly once.
+ * The partial K psi of the received block goes back to its owner, E_x is summed over ranks.
+ */
+exx_status exx_round_robin_step(int n_ranks, int rank, int step, int *send_to, int *recv_from, int *what);
 
 /*
  * exx_schedule_pairs -- HOST-only view of the pair scheduler (no GPU needed): the number of Poisson solves
@@ -111,6 +179,13 @@ exx_status exx_schedule_pairs(int n_orb, const double *occ_host, long long *n_pa
  */
 exx_status exx_schedule_list(int n_orb, const double *occ_host, int max_batch, int *xforms_host, long long capacity,
                              long long *n_transforms);
+/* The same listing for exx_apply_pairs (pair_mask_host as there; NULL = no mask) and for the rectangular blocks of
+ * exx_apply_block (occ_res_host != NULL) / exx_apply_to (occ_res_host == NULL: streamed orbitals with f = 0 skipped):
+ * j, l index the resident set, i the streamed set. */
+exx_status exx_schedule_list_masked(int n_orb, const double *occ_host, const unsigned char *pair_mask_host, int max_batch,
+                                    int *xforms_host, long long capacity, long long *n_transforms);
+exx_status exx_schedule_list_block(int n_res, const double *occ_res_host, int n_str, const double *occ_str_host,
+                                   int max_batch, int *xforms_host, long long capacity, long long *n_transforms);
 
 /* Transform-grid lengths (n or 2n) of a plan and the bytes of device workspace it owns. */
 exx_status exx_plan_transform_dims(const exx_plan *plan, int tdims[3]);
@@ -122,6 +197,11 @@ const char *exx_plan_kernel_name(const exx_plan *plan, int pass);
 
 /* Number of kernel launches the library has enqueued for this plan since creation (for bench "gpu_launches"). */
 long long  exx_plan_launch_count(const exx_plan *plan);
+
+/* Ordinal of the CUDA device the plan lives on (the device that was current in exx_plan_create; the stream passed there
+ * must belong to it).  Every entry point makes that device current for the duration of the call and restores the
+ * caller's, so plans on different GPUs can be driven from one host thread.  -1 for NULL. */
+int        exx_plan_device(const exx_plan *plan);
 
 /*
  * Per-pass device timing (CUDA events on the plan's stream around every pass launch).  Off by default.

@@ -36,6 +36,10 @@ def _load():
         lib.exx_oracle_realspace_kernel.argtypes = [C.c_void_p, _dp]
         lib.exx_oracle_poisson_direct.argtypes = [C.c_void_p, _dp, _dp]
         lib.exx_oracle_kpsi_points.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int, _ip, _lp, _dp]
+        lib.exx_oracle_apply_masked.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_void_p, _dp, _dp, _dp]
+        lib.exx_oracle_apply_to.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int, _dp, _dp]
+        lib.exx_oracle_apply_block.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp]
+        lib.exx_oracle_set_periodic_filter.argtypes = [C.c_void_p, _dp]
         lib.exx_oracle_threads.argtypes = []
         _lib = lib
     return _lib
@@ -63,6 +67,8 @@ class Oracle:
     """Plain CPU exact-exchange oracle for one grid / boundary condition / Green's function."""
 
     def __init__(self, dims, spacing, bc, kernel=None):
+        """kernel: free BC -> real-space table g[n1][n2][n3]; periodic BC -> None (analytic 4 pi/|G|^2) or a
+        Fourier-space filter table on the symmetric index range [n1/2+1][n2/2+1][n3/2+1]."""
         lib = _load()
         self.dims = tuple(int(d) for d in dims)
         self.spacing = tuple(float(h) for h in spacing)
@@ -72,14 +78,21 @@ class Oracle:
         d = (C.c_int * 3)(*self.dims)
         h = (C.c_double * 3)(*self.spacing)
         k = None
-        if kernel is not None:
+        filt = None
+        if kernel is not None and self.bc == 1:
             k = _f64(kernel)
             if k.size != self.M:
                 raise ValueError("kernel table must have n1*n2*n3 entries")
+        elif kernel is not None:
+            filt = _f64(kernel)
+            if filt.size != (self.dims[0] // 2 + 1) * (self.dims[1] // 2 + 1) * (self.dims[2] // 2 + 1):
+                raise ValueError("periodic filter table must have (n1/2+1)(n2/2+1)(n3/2+1) entries")
         self._h = C.c_void_p()
         rc = lib.exx_oracle_create(C.byref(self._h), d, h, self.bc, _d(k) if k is not None else None)
         if rc:
             raise RuntimeError(f"exx_oracle_create failed ({rc})")
+        if filt is not None and lib.exx_oracle_set_periodic_filter(self._h, _d(filt)):
+            raise RuntimeError("exx_oracle_set_periodic_filter failed")
         t = (C.c_int * 3)()
         lib.exx_oracle_transform_dims(self._h, t)
         self.tdims = tuple(t)
@@ -139,6 +152,54 @@ class Oracle:
         if rc:
             raise RuntimeError(f"exx_oracle_apply failed ({rc})")
         return kpsi.reshape((n_orb,) + self.dims), ex.value, e
+
+    def apply_masked(self, psi, occ, mask):
+        """As apply() with the ordered pairs whose mask entry is 0 left out.  Returns (kpsi, E_x, e_pair)."""
+        psi = _f64(psi)
+        n_orb = psi.shape[0]
+        psi = psi.reshape(n_orb, self.M)
+        occ = _f64(occ)
+        m = np.ascontiguousarray((np.asarray(mask) != 0).astype(np.uint8))
+        if m.shape != (n_orb, n_orb):
+            raise ValueError("mask must have shape (n_orb, n_orb)")
+        kpsi = np.empty_like(psi)
+        ex = C.c_double()
+        e = np.empty((n_orb, n_orb))
+        rc = _load().exx_oracle_apply_masked(self._h, n_orb, _d(psi), _d(occ), C.c_void_p(m.ctypes.data), _d(kpsi), C.byref(ex), _d(e))
+        if rc:
+            raise RuntimeError(f"exx_oracle_apply_masked failed ({rc})")
+        return kpsi.reshape((n_orb,) + self.dims), ex.value, e
+
+    def apply_to(self, psi, occ, phi):
+        """K of the occupied set (psi, occ) applied to phi: returns kphi[n_tgt, n1, n2, n3]."""
+        psi = _f64(psi)
+        phi = _f64(phi)
+        n_occ, n_tgt = psi.shape[0], phi.shape[0]
+        psi = psi.reshape(n_occ, self.M)
+        phi = phi.reshape(n_tgt, self.M)
+        occ = _f64(occ)
+        kphi = np.empty_like(phi)
+        rc = _load().exx_oracle_apply_to(self._h, n_occ, _d(psi), _d(occ), n_tgt, _d(phi), _d(kphi))
+        if rc:
+            raise RuntimeError(f"exx_oracle_apply_to failed ({rc})")
+        return kphi.reshape((n_tgt,) + self.dims)
+
+    def apply_block(self, psi_a, occ_a, psi_b, occ_b):
+        """All pairs between two disjoint blocks: returns (ka, kb, ex, e_block[n_a, n_b])."""
+        psi_a = _f64(psi_a)
+        psi_b = _f64(psi_b)
+        n_a, n_b = psi_a.shape[0], psi_b.shape[0]
+        psi_a = psi_a.reshape(n_a, self.M)
+        psi_b = psi_b.reshape(n_b, self.M)
+        occ_a, occ_b = _f64(occ_a), _f64(occ_b)
+        ka, kb = np.empty_like(psi_a), np.empty_like(psi_b)
+        ex = C.c_double()
+        e = np.empty((n_a, n_b))
+        rc = _load().exx_oracle_apply_block(self._h, n_a, _d(psi_a), _d(occ_a), _d(ka), n_b, _d(psi_b), _d(occ_b), _d(kb),
+                                            C.byref(ex), _d(e))
+        if rc:
+            raise RuntimeError(f"exx_oracle_apply_block failed ({rc})")
+        return ka.reshape((n_a,) + self.dims), kb.reshape((n_b,) + self.dims), ex.value, e
 
     def rows(self, psi, occ, rows):
         """Complete rows K psi_i for listed i: returns (kpsi_rows[len(rows),n1,n2,n3], e_rows[len(rows),N])."""

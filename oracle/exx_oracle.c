@@ -235,6 +235,29 @@ int exx_oracle_create(exx_oracle **out, const int dims[3], const double spacing[
     return 0;
 }
 
+/* PERIODIC only: replace the analytic Coulomb kernel by a host-supplied Fourier-space filter ("only the filter F of
+ * kernel 2 would be different", PAPER.md:236 -- screened hybrids): table[s0][s1][s2] on the symmetric index range
+ * s_ax = 0..t_ax/2, frequency index m = a if 2a <= t else a - t, K^(a,b,c) = table[|ma|][|mb|][|mc|]. */
+int exx_oracle_set_periodic_filter(exx_oracle *o, const double *table)
+{
+    if (!o || !table || o->bc != EXX_ORACLE_PERIODIC) return 1;
+    const int t0 = o->t[0], t1 = o->t[1], t2 = o->t[2];
+    const int s1 = t1 / 2 + 1, s2 = t2 / 2 + 1;
+    for (int a = 0; a < t0; ++a) {
+        int ma = (2 * a <= t0) ? a : t0 - a;
+        for (int b = 0; b < t1; ++b) {
+            int mb = (2 * b <= t1) ? b : t1 - b;
+            for (int c = 0; c < t2; ++c) {
+                int mc = (2 * c <= t2) ? c : t2 - c;
+                cplx *k = &o->khat[((long long)a * t1 + b) * t2 + c];
+                k->re = table[((long long)ma * s1 + mb) * s2 + mc];
+                k->im = 0.0;
+            }
+        }
+    }
+    return 0;
+}
+
 void exx_oracle_destroy(exx_oracle *o)
 {
     if (!o) return;
@@ -317,9 +340,11 @@ static double pair_energy(const exx_oracle *o, const double *rho, const double *
  *   E_x    -= 1/2 f_i f_j e_ij (Eq. 2 / :81-82 Eq. 5, reading A4: one channel, f as passed)
  * OpenMP over the target orbital i: the owner computes Kpsi_i, no shared writes.
  * ------------------------------------------------------------------------------------------------- */
-int exx_oracle_apply(const exx_oracle *o, int n_orb, const double *psi, const double *occ,
-                     double *kpsi, double *ex, double *e_pair, int symmetric)
+static int apply_pairs(const exx_oracle *o, int n_orb, const double *psi, const double *occ, const unsigned char *mask,
+                       double *kpsi, double *ex, double *e_pair, int symmetric)
 {
+    /* mask (optional, [n_orb][n_orb]): the ordered pair (i,j) is left out of every sum when mask[i][j] == 0
+     * (localised orbitals: co-densities of orbitals that do not overlap vanish). */
     if (!o || n_orb <= 0 || !psi || !occ || !kpsi || !ex) return 1;
     const long long M = o->M;
     memset(kpsi, 0, sizeof(double) * (size_t)M * n_orb);
@@ -347,6 +372,7 @@ int exx_oracle_apply(const exx_oracle *o, int n_orb, const double *psi, const do
                     double *ki = kpsi + (long long)i * M;
                     for (int j = 0; j < n_orb; ++j) {
                         const double *pj = psi + (long long)j * M;
+                        if (mask && !mask[(long long)i * n_orb + j]) continue;
                         for (long long r = 0; r < M; ++r) rho[r] = pi[r] * pj[r];          /* Eq. 8 */
                         if (poisson_work(o, rho, v, work)) {                              /* Eq. 4 */
 #pragma omp atomic write
@@ -396,6 +422,7 @@ int exx_oracle_apply(const exx_oracle *o, int n_orb, const double *psi, const do
                         const double *pj = psi + (long long)j * M;
                         const double fj = occ[j];
                         if (fi == 0.0 && fj == 0.0) continue;                             /* A15 */
+                        if (mask && !mask[(long long)i * n_orb + j]) continue;
                         for (long long r = 0; r < M; ++r) rho[r] = pi[r] * pj[r];
                         if (poisson_work(o, rho, v, work)) {
 #pragma omp atomic write
@@ -432,6 +459,145 @@ int exx_oracle_apply(const exx_oracle *o, int n_orb, const double *psi, const do
             ksum_add(&k, -0.5 * occ[i] * occ[j] * e_mat[(long long)i * n_orb + j]);
     *ex = ksum_get(&k);
     if (e_pair) memcpy(e_pair, e_mat, sizeof(double) * (size_t)n_orb * n_orb);
+    free(e_mat);
+    return 0;
+}
+
+int exx_oracle_apply(const exx_oracle *o, int n_orb, const double *psi, const double *occ,
+                     double *kpsi, double *ex, double *e_pair, int symmetric)
+{
+    return apply_pairs(o, n_orb, psi, occ, NULL, kpsi, ex, e_pair, symmetric);
+}
+
+int exx_oracle_apply_masked(const exx_oracle *o, int n_orb, const double *psi, const double *occ,
+                            const unsigned char *mask, double *kpsi, double *ex, double *e_pair)
+{
+    if (!mask) return 1;
+    return apply_pairs(o, n_orb, psi, occ, mask, kpsi, ex, e_pair, 0);
+}
+
+/* ---------------------------------------------------------------------------------------------------
+ * The exchange operator built from the occupied set (psi_j, f_j) applied to another orbital set phi_t
+ * (Eq. 3 with phi_t in the place of psi_i; unoccupied states and the second spin channel of the
+ * paper's runs):   Kphi_t = - sum_j f_j V[phi_t psi_j] psi_j.   OpenMP over t.
+ * ------------------------------------------------------------------------------------------------- */
+int exx_oracle_apply_to(const exx_oracle *o, int n_occ, const double *psi, const double *occ,
+                        int n_tgt, const double *phi, double *kphi)
+{
+    if (!o || n_occ <= 0 || n_tgt <= 0 || !psi || !occ || !phi || !kphi) return 1;
+    const long long M = o->M;
+    memset(kphi, 0, sizeof(double) * (size_t)M * n_tgt);
+    int fail = 0;
+#ifdef _OPENMP
+    g_threads_used = omp_get_max_threads();
+#endif
+#pragma omp parallel
+    {
+        cplx *work = (cplx *)malloc(sizeof(cplx) * (size_t)o->T);
+        double *rho = (double *)malloc(sizeof(double) * (size_t)M);
+        double *v = (double *)malloc(sizeof(double) * (size_t)M);
+        if (!work || !rho || !v) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(dynamic, 1)
+            for (int t = 0; t < n_tgt; ++t) {
+                const double *pt = phi + (long long)t * M;
+                double *kt = kphi + (long long)t * M;
+                for (int j = 0; j < n_occ; ++j) {
+                    const double *pj = psi + (long long)j * M;
+                    for (long long r = 0; r < M; ++r) rho[r] = pt[r] * pj[r];             /* Eq. 8 */
+                    if (poisson_work(o, rho, v, work)) {                                  /* Eq. 4 */
+#pragma omp atomic write
+                        fail = 1;
+                        continue;
+                    }
+                    const double fj = occ[j];
+                    for (long long r = 0; r < M; ++r) kt[r] -= fj * v[r] * pj[r];          /* Eq. 3 */
+                }
+            }
+        }
+        free(work); free(rho); free(v);
+    }
+    return fail ? 2 : 0;
+}
+
+/* ---------------------------------------------------------------------------------------------------
+ * All pairs between two DISJOINT orbital blocks A (n_a orbitals) and B (n_b): the unit of work of the paper's
+ * round-robin distribution (Fig. 1).  Written from each owner's point of view, every potential
+ * solved separately for the two sides (no reuse of V_ab for V_ba):
+ *   ka[a] = - sum_b f_b V_ab psi_b      kb[b] = - sum_a f_a V_ba psi_a      e[a][b] = dV sum_r rho_ab V_ab
+ *   ex    = - sum_{a,b} f_a f_b e_ab    (Eq. 5 counts the ordered pairs (a,b) and (b,a): 2 * (-1/2))
+ * ka, kb are OVERWRITTEN.
+ * ------------------------------------------------------------------------------------------------- */
+int exx_oracle_apply_block(const exx_oracle *o, int n_a, const double *psi_a, const double *occ_a, double *ka,
+                           int n_b, const double *psi_b, const double *occ_b, double *kb, double *ex, double *e_block)
+{
+    if (!o || n_a <= 0 || n_b <= 0 || !psi_a || !occ_a || !ka || !psi_b || !occ_b || !kb || !ex) return 1;
+    const long long M = o->M;
+    memset(ka, 0, sizeof(double) * (size_t)M * n_a);
+    memset(kb, 0, sizeof(double) * (size_t)M * n_b);
+    double *e_mat = (double *)calloc((size_t)n_a * n_b, sizeof(double));
+    if (!e_mat) return 2;
+    int fail = 0;
+#ifdef _OPENMP
+    g_threads_used = omp_get_max_threads();
+#endif
+#pragma omp parallel
+    {
+        cplx *work = (cplx *)malloc(sizeof(cplx) * (size_t)o->T);
+        double *rho = (double *)malloc(sizeof(double) * (size_t)M);
+        double *v = (double *)malloc(sizeof(double) * (size_t)M);
+        if (!work || !rho || !v) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(dynamic, 1)
+            for (int a = 0; a < n_a; ++a) {                              /* side A receives from every b */
+                const double *pa = psi_a + (long long)a * M;
+                double *k = ka + (long long)a * M;
+                for (int b = 0; b < n_b; ++b) {
+                    const double *pb = psi_b + (long long)b * M;
+                    for (long long r = 0; r < M; ++r) rho[r] = pa[r] * pb[r];
+                    if (poisson_work(o, rho, v, work)) {
+#pragma omp atomic write
+                        fail = 1;
+                        continue;
+                    }
+                    const double fb = occ_b[b];
+                    for (long long r = 0; r < M; ++r) k[r] -= fb * v[r] * pb[r];
+                    e_mat[(long long)a * n_b + b] = pair_energy(o, rho, v);
+                }
+            }
+#pragma omp for schedule(dynamic, 1)
+            for (int b = 0; b < n_b; ++b) {                              /* side B receives from every a */
+                const double *pb = psi_b + (long long)b * M;
+                double *k = kb + (long long)b * M;
+                for (int a = 0; a < n_a; ++a) {
+                    const double *pa = psi_a + (long long)a * M;
+                    for (long long r = 0; r < M; ++r) rho[r] = pb[r] * pa[r];
+                    if (poisson_work(o, rho, v, work)) {
+#pragma omp atomic write
+                        fail = 1;
+                        continue;
+                    }
+                    const double fa = occ_a[a];
+                    for (long long r = 0; r < M; ++r) k[r] -= fa * v[r] * pa[r];
+                }
+            }
+        }
+        free(work); free(rho); free(v);
+    }
+    if (fail) { free(e_mat); return 2; }
+    ksum k = { 0.0, 0.0 };
+    for (int a = 0; a < n_a; ++a)
+        for (int b = 0; b < n_b; ++b) ksum_add(&k, -occ_a[a] * occ_b[b] * e_mat[(long long)a * n_b + b]);
+    *ex = ksum_get(&k);
+    if (e_block) memcpy(e_block, e_mat, sizeof(double) * (size_t)n_a * n_b);
     free(e_mat);
     return 0;
 }

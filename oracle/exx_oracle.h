@@ -17,7 +17,9 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): P1 FFT vs direct DFT; P2/P3 brute-force O(M^2) real-space
  * convolution on tiny grids (free / periodic); P4/P5 plane-wave closed forms; P6 Gaussian -> erf(r/(sqrt2 s))/r;
  * P7 symmetry invariants; P8 energy/operator consistency incl. finite differences; P9 N=1 Hartree, index-n plane;
- * P10 Table 1 pair counts.  Parity unpinned: none.
+ * P10 Table 1 pair counts; P11 apply_to (coincident sets, two-cosine closed form, linearity, symmetry); P12 apply_block
+ * (union of two sets = parts + block); P13 masked apply (all-ones mask, block-diagonal mask = independent subsystems);
+ * P14 periodic filter table (Coulomb table = analytic kernel, screened plane-wave closed form).  Parity unpinned: none.
  *
  * All pointers are HOST pointers.  Arrays are C order, psi[i][a][b][c], last index fastest.
  * Return value: 0 on success, non-zero on invalid arguments / allocation failure.
@@ -55,6 +57,26 @@ int exx_oracle_poisson(const exx_oracle *o, const double *rho, double *v);
  * exists to make long runs affordable and is itself validated against symmetric=0 in the tests. */
 int exx_oracle_apply(const exx_oracle *o, int n_orb, const double *psi, const double *occ,
                      double *kpsi, double *ex, double *e_pair, int symmetric);
+
+/* As exx_oracle_apply (symmetric=0) with the ordered pairs (i,j) whose mask[i*n_orb+j] == 0 left out of every sum
+ * (localised orbitals, Eq. 6-7). */
+int exx_oracle_apply_masked(const exx_oracle *o, int n_orb, const double *psi, const double *occ,
+                            const unsigned char *mask, double *kpsi, double *ex, double *e_pair);
+
+/* K of the occupied set (psi, occ) applied to another set: kphi[t] = - sum_j f_j V[phi_t psi_j] psi_j
+ * (PAPER.md:67-69 Eq. 3; :210, :244 unoccupied states / second spin channel).  kphi (n_tgt*M) is OVERWRITTEN. */
+int exx_oracle_apply_to(const exx_oracle *o, int n_occ, const double *psi, const double *occ,
+                        int n_tgt, const double *phi, double *kphi);
+
+/* All pairs between two disjoint blocks A and B (the round-robin unit of work): ka[a] = -sum_b f_b
+ * V_ab psi_b, kb[b] = -sum_a f_a V_ba psi_a (both OVERWRITTEN), e_block[a][b] = e_ab (may be NULL),
+ * *ex = -sum_ab f_a f_b e_ab. */
+int exx_oracle_apply_block(const exx_oracle *o, int n_a, const double *psi_a, const double *occ_a, double *ka,
+                           int n_b, const double *psi_b, const double *occ_b, double *kb, double *ex, double *e_block);
+
+/* PERIODIC only: use the host table K^[s0][s1][s2] (symmetric index range s = 0..t/2 per axis, even in every index)
+ * instead of 4 pi/|G|^2 (screened hybrids change only this filter). */
+int exx_oracle_set_periodic_filter(exx_oracle *o, const double *table);
 
 /* Complete rows: for each listed i, Kpsi_i (all j) into kpsi_rows[row][M] and e_ij into e_rows[row][N] (may be NULL). */
 int exx_oracle_rows(const exx_oracle *o, int n_orb, const double *psi, const double *occ,

@@ -20,9 +20,13 @@ EXX_BC_PERIODIC, EXX_BC_FREE = 0, 1
 _STATUS = ["EXX_OK", "EXX_ERR_INVALID_ARG", "EXX_ERR_UNSUPPORTED_SIZE", "EXX_ERR_BAD_POINTER", "EXX_ERR_ALLOC",
            "EXX_ERR_CUDA", "EXX_ERR_INTERNAL"]
 
+EXX_BLOCK_ACCUMULATE_RESIDENT, EXX_BLOCK_ACCUMULATE_STREAMED = 1, 2
+
 EXPORTS = [
-    "exx_plan_create", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_get_pair_energies",
-    "exx_schedule_pairs", "exx_schedule_list", "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_kernel_name",
+    "exx_plan_create", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_apply_pairs", "exx_apply_to", "exx_apply_block",
+    "exx_get_pair_energies", "exx_get_block_energies", "exx_plan_release_staging",
+    "exx_schedule_pairs", "exx_schedule_list", "exx_schedule_list_masked", "exx_schedule_list_block", "exx_round_robin_step",
+    "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_device", "exx_plan_kernel_name",
     "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version",
 ]
 
@@ -56,8 +60,27 @@ def load_library():
         fn = getattr(lib, name)
         fn.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_void_p]
         fn.restype = C.c_int
-    lib.exx_get_pair_energies.argtypes = [C.c_void_p, _dp]
+    lib.exx_get_pair_energies.argtypes = [C.c_void_p, C.c_int, _dp]
     lib.exx_get_pair_energies.restype = C.c_int
+    lib.exx_get_block_energies.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
+    lib.exx_get_block_energies.restype = C.c_int
+    lib.exx_plan_release_staging.argtypes = [C.c_void_p]
+    lib.exx_plan_release_staging.restype = C.c_int
+    lib.exx_apply_pairs.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.exx_apply_pairs.restype = C.c_int
+    lib.exx_apply_to.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_int, C.c_void_p, C.c_void_p]
+    lib.exx_apply_to.restype = C.c_int
+    lib.exx_apply_block.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_int,
+                                    C.c_void_p]
+    lib.exx_apply_block.restype = C.c_int
+    lib.exx_schedule_list_masked.argtypes = [C.c_int, _dp, C.c_void_p, C.c_int, _ip, C.c_longlong, C.POINTER(C.c_longlong)]
+    lib.exx_schedule_list_masked.restype = C.c_int
+    lib.exx_schedule_list_block.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_int, _ip, C.c_longlong, C.POINTER(C.c_longlong)]
+    lib.exx_schedule_list_block.restype = C.c_int
+    lib.exx_round_robin_step.argtypes = [C.c_int, C.c_int, C.c_int, _ip, _ip, _ip]
+    lib.exx_round_robin_step.restype = C.c_int
+    lib.exx_plan_device.argtypes = [C.c_void_p]
+    lib.exx_plan_device.restype = C.c_int
     lib.exx_schedule_pairs.argtypes = [C.c_int, _dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     lib.exx_schedule_pairs.restype = C.c_int
     lib.exx_schedule_list.argtypes = [C.c_int, _dp, C.c_int, _ip, C.c_longlong, C.POINTER(C.c_longlong)]
@@ -102,20 +125,60 @@ def exx_schedule_pairs(occ: Sequence[float]):
     return n_pairs.value, n_x.value
 
 
-def exx_schedule_list(occ: Sequence[float], max_batch: int = 0):
-    """int32 array [n_transforms][5] of {j, l, i, flags, batch} -- host only, no GPU needed (see include/exx.h)."""
+def _mask_array(mask, n_orb: int) -> np.ndarray:
+    m = np.ascontiguousarray((np.asarray(mask) != 0).astype(np.uint8))
+    if m.shape != (n_orb, n_orb):
+        raise ValueError("pair mask must have shape (n_orb, n_orb)")
+    return m
+
+
+def exx_schedule_list(occ: Sequence[float], max_batch: int = 0, pair_mask=None):
+    """int32 array [n_transforms][5] of {j, l, i, flags, batch} -- host only, no GPU needed (see include/exx.h).
+    pair_mask: optional (n_orb, n_orb) symmetric mask of the pairs to solve (exx_schedule_list_masked)."""
     occ = np.ascontiguousarray(np.asarray(occ, dtype=np.float64))
     lib = load_library()
     n_x = C.c_longlong()
-    st = lib.exx_schedule_list(int(occ.size), occ.ctypes.data_as(_dp), int(max_batch), None, 0, C.byref(n_x))
-    if st:
-        raise ExxError(st, "exx_schedule_list")
-    out = np.zeros((n_x.value, 5), dtype=np.int32)
-    if n_x.value:
-        st = lib.exx_schedule_list(int(occ.size), occ.ctypes.data_as(_dp), int(max_batch), out.ctypes.data_as(_ip), n_x.value, C.byref(n_x))
+    m = _mask_array(pair_mask, occ.size) if pair_mask is not None else None
+    mp = C.c_void_p(m.ctypes.data) if m is not None else None
+
+    def call(buf, cap):
+        st = lib.exx_schedule_list_masked(int(occ.size), occ.ctypes.data_as(_dp), mp, int(max_batch), buf, cap, C.byref(n_x))
         if st:
             raise ExxError(st, "exx_schedule_list")
+    call(None, 0)
+    out = np.zeros((n_x.value, 5), dtype=np.int32)
+    if n_x.value:
+        call(out.ctypes.data_as(_ip), n_x.value)
     return out
+
+
+def exx_schedule_list_block(occ_res, occ_str: Sequence[float], n_res: Optional[int] = None, max_batch: int = 0):
+    """Listing of the rectangular schedule of exx_apply_block (occ_res given) or exx_apply_to (occ_res None, n_res given)."""
+    occ_str = np.ascontiguousarray(np.asarray(occ_str, dtype=np.float64))
+    occ_r = None if occ_res is None else np.ascontiguousarray(np.asarray(occ_res, dtype=np.float64))
+    n_res = int(occ_r.size) if occ_r is not None else int(n_res)
+    lib = load_library()
+    n_x = C.c_longlong()
+
+    def call(buf, cap):
+        st = lib.exx_schedule_list_block(n_res, occ_r.ctypes.data_as(_dp) if occ_r is not None else None, int(occ_str.size),
+                                         occ_str.ctypes.data_as(_dp), int(max_batch), buf, cap, C.byref(n_x))
+        if st:
+            raise ExxError(st, "exx_schedule_list_block")
+    call(None, 0)
+    out = np.zeros((n_x.value, 5), dtype=np.int32)
+    if n_x.value:
+        call(out.ctypes.data_as(_ip), n_x.value)
+    return out
+
+
+def exx_round_robin_step(n_ranks: int, rank: int, step: int):
+    """(send_to, recv_from, what) of step `step` of the round-robin block exchange (include/exx.h) -- host only."""
+    a, b, w = C.c_int(), C.c_int(), C.c_int()
+    st = load_library().exx_round_robin_step(int(n_ranks), int(rank), int(step), C.byref(a), C.byref(b), C.byref(w))
+    if st:
+        raise ExxError(st, "exx_round_robin_step")
+    return a.value, b.value, w.value
 
 
 class ExxPlan:
@@ -132,8 +195,12 @@ class ExxPlan:
         kptr = None
         if kernel is not None:
             self._kernel = np.ascontiguousarray(np.asarray(kernel, dtype=np.float64))
-            if self._kernel.size != self.dims[0] * self.dims[1] * self.dims[2]:
-                raise ValueError("kernel table must have n1*n2*n3 entries")
+            if self.bc == EXX_BC_FREE:
+                want = self.dims[0] * self.dims[1] * self.dims[2]
+            else:                                       # periodic: Fourier-space filter on the symmetric index range
+                want = (self.dims[0] // 2 + 1) * (self.dims[1] // 2 + 1) * (self.dims[2] // 2 + 1)
+            if self._kernel.size != want:
+                raise ValueError(f"kernel table must have {want} entries for this boundary condition")
             kptr = self._kernel.ctypes.data_as(_dp)
         self._h = C.c_void_p()
         st = lib.exx_plan_create(C.byref(self._h), d, h, self.bc, kptr, self.max_orbitals,
@@ -178,47 +245,126 @@ class ExxPlan:
         self._check(load_library().exx_plan_get_profile(self._h, ms, n))
         return list(ms), list(n)
 
-    # -- the hot path
-    def apply(self, psi, occ, kpsi=None):
-        """exx_apply: returns (kpsi, E_x).  psi/kpsi are CUDA tensors (data_ptr is handed to the library)."""
+    # -- argument checks of the binding (shape / dtype / residency; the library re-checks pointers, alignment, overlap)
+    def _check_dev(self, t, name, n_orb=None):
         import torch
-        if not (psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous()):
-            raise ValueError("psi must be a contiguous CUDA float64 tensor")
-        if tuple(psi.shape[1:]) != self.dims:
-            raise ValueError("psi grid shape does not match the plan")
-        if kpsi is None:
-            kpsi = torch.empty_like(psi)
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA float64 tensor")
+        if t.dim() != 4 or tuple(t.shape[1:]) != self.dims:
+            raise ValueError(f"{name} must have shape (N, {self.dims[0]}, {self.dims[1]}, {self.dims[2]})")
+        if n_orb is not None and t.shape[0] != n_orb:
+            raise ValueError(f"{name} must hold {n_orb} orbitals")
+        if t.device.index != self.device:
+            raise ValueError(f"{name} lives on cuda:{t.device.index}, the plan on cuda:{self.device}")
+        return t
+
+    @staticmethod
+    def _occ(occ, n_orb, name="occ"):
         occ = np.ascontiguousarray(np.asarray(occ, dtype=np.float64))
+        if occ.ndim != 1 or occ.size != n_orb:
+            raise ValueError(f"{name} must hold one occupation per orbital ({n_orb})")
+        return occ
+
+    @property
+    def device(self) -> int:
+        return int(load_library().exx_plan_device(self._h))
+
+    # -- the hot path
+    def apply(self, psi, occ, kpsi=None, pair_mask=None):
+        """exx_apply (or exx_apply_pairs with a pair mask): returns (kpsi, E_x).  psi/kpsi are CUDA tensors whose
+        data_ptr is handed to the library."""
+        import torch
+        self._check_dev(psi, "psi")
+        n_orb = int(psi.shape[0])
+        kpsi = torch.empty_like(psi) if kpsi is None else self._check_dev(kpsi, "kpsi", n_orb)
+        occ = self._occ(occ, n_orb)
         ex = C.c_double()
-        st = load_library().exx_apply(self._h, int(psi.shape[0]), C.c_void_p(psi.data_ptr()), occ.ctypes.data_as(_dp),
-                                      C.c_void_p(kpsi.data_ptr()), C.cast(C.byref(ex), C.c_void_p))
+        lib = load_library()
+        if pair_mask is None:
+            st = lib.exx_apply(self._h, n_orb, C.c_void_p(psi.data_ptr()), occ.ctypes.data_as(_dp), C.c_void_p(kpsi.data_ptr()),
+                               C.cast(C.byref(ex), C.c_void_p))
+        else:
+            m = _mask_array(pair_mask, n_orb)
+            st = lib.exx_apply_pairs(self._h, n_orb, C.c_void_p(psi.data_ptr()), occ.ctypes.data_as(_dp), C.c_void_p(m.ctypes.data),
+                                     C.c_void_p(kpsi.data_ptr()), C.cast(C.byref(ex), C.c_void_p))
         self._check(st)
+        self._last_n_orb = n_orb
         return kpsi, ex.value
 
     def apply_async(self, psi, occ, kpsi, ex_dev):
         """exx_apply_async: no synchronisation, E_x lands in the 1-element CUDA tensor ex_dev."""
-        occ = np.ascontiguousarray(np.asarray(occ, dtype=np.float64))
-        st = load_library().exx_apply_async(self._h, int(psi.shape[0]), C.c_void_p(psi.data_ptr()), occ.ctypes.data_as(_dp),
+        import torch
+        self._check_dev(psi, "psi")
+        n_orb = int(psi.shape[0])
+        self._check_dev(kpsi, "kpsi", n_orb)
+        if not (isinstance(ex_dev, torch.Tensor) and ex_dev.is_cuda and ex_dev.dtype == torch.float64 and ex_dev.numel() >= 1):
+            raise ValueError("ex_dev must be a CUDA float64 tensor with at least one element")
+        occ = self._occ(occ, n_orb)
+        st = load_library().exx_apply_async(self._h, n_orb, C.c_void_p(psi.data_ptr()), occ.ctypes.data_as(_dp),
                                             C.c_void_p(kpsi.data_ptr()), C.c_void_p(ex_dev.data_ptr()))
         self._check(st)
+        self._last_n_orb = n_orb
 
     def apply_host(self, psi_host: np.ndarray, occ, kpsi_host: Optional[np.ndarray] = None):
         """exx_apply_host: host buffers in, host buffers out (copies inside the library)."""
-        if not (psi_host.dtype == np.float64 and psi_host.flags.c_contiguous):
-            raise ValueError("psi_host must be C-contiguous float64")
+        if not (psi_host.dtype == np.float64 and psi_host.flags.c_contiguous and psi_host.ndim == 4 and tuple(psi_host.shape[1:]) == self.dims):
+            raise ValueError("psi_host must be C-contiguous float64 of shape (N, n1, n2, n3)")
         if kpsi_host is None:
             kpsi_host = np.empty_like(psi_host)
-        occ = np.ascontiguousarray(np.asarray(occ, dtype=np.float64))
+        elif not (kpsi_host.dtype == np.float64 and kpsi_host.flags.c_contiguous and kpsi_host.shape == psi_host.shape and kpsi_host.flags.writeable):
+            raise ValueError("kpsi_host must be writable C-contiguous float64 with the shape of psi_host")
+        n_orb = int(psi_host.shape[0])
+        occ = self._occ(occ, n_orb)
         ex = C.c_double()
-        st = load_library().exx_apply_host(self._h, int(psi_host.shape[0]), C.c_void_p(psi_host.ctypes.data),
-                                           occ.ctypes.data_as(_dp), C.c_void_p(kpsi_host.ctypes.data),
-                                           C.cast(C.byref(ex), C.c_void_p))
+        st = load_library().exx_apply_host(self._h, n_orb, C.c_void_p(psi_host.ctypes.data), occ.ctypes.data_as(_dp),
+                                           C.c_void_p(kpsi_host.ctypes.data), C.cast(C.byref(ex), C.c_void_p))
         self._check(st)
+        self._last_n_orb = n_orb
         return kpsi_host, ex.value
 
-    def pair_energies(self, n_orb: int) -> np.ndarray:
+    def release_staging(self):
+        self._check(load_library().exx_plan_release_staging(self._h))
+
+    def apply_to(self, psi, occ, phi, kphi=None):
+        """exx_apply_to: K (built from the occupied psi, occ) applied to the orbitals phi; returns kphi."""
+        import torch
+        self._check_dev(psi, "psi")
+        self._check_dev(phi, "phi")
+        kphi = torch.empty_like(phi) if kphi is None else self._check_dev(kphi, "kphi", int(phi.shape[0]))
+        occ = self._occ(occ, int(psi.shape[0]))
+        st = load_library().exx_apply_to(self._h, int(psi.shape[0]), C.c_void_p(psi.data_ptr()), occ.ctypes.data_as(_dp),
+                                         int(phi.shape[0]), C.c_void_p(phi.data_ptr()), C.c_void_p(kphi.data_ptr()))
+        self._check(st)
+        return kphi
+
+    def apply_block(self, psi_res, occ_res, kpsi_res, psi_str, occ_str, kpsi_str, flags=0):
+        """exx_apply_block: all pairs between two disjoint blocks; returns the block's contribution to E_x."""
+        self._check_dev(psi_res, "psi_res")
+        self._check_dev(psi_str, "psi_str")
+        self._check_dev(kpsi_res, "kpsi_res", int(psi_res.shape[0]))
+        self._check_dev(kpsi_str, "kpsi_str", int(psi_str.shape[0]))
+        occ_res = self._occ(occ_res, int(psi_res.shape[0]), "occ_res")
+        occ_str = self._occ(occ_str, int(psi_str.shape[0]), "occ_str")
+        ex = C.c_double()
+        st = load_library().exx_apply_block(self._h, int(psi_res.shape[0]), C.c_void_p(psi_res.data_ptr()), occ_res.ctypes.data_as(_dp),
+                                            C.c_void_p(kpsi_res.data_ptr()), int(psi_str.shape[0]), C.c_void_p(psi_str.data_ptr()),
+                                            occ_str.ctypes.data_as(_dp), C.c_void_p(kpsi_str.data_ptr()), int(flags),
+                                            C.cast(C.byref(ex), C.c_void_p))
+        self._check(st)
+        return ex.value
+
+    def pair_energies(self, n_orb: Optional[int] = None) -> np.ndarray:
+        """e_ij of the most recent square apply; n_orb defaults to that apply's orbital count (the library checks it)."""
+        n_orb = int(n_orb if n_orb is not None else getattr(self, "_last_n_orb", 0))
+        if n_orb < 1:
+            raise ValueError("no apply has run on this plan")
         e = np.empty((n_orb, n_orb))
-        self._check(load_library().exx_get_pair_energies(self._h, e.ctypes.data_as(_dp)))
+        self._check(load_library().exx_get_pair_energies(self._h, n_orb, e.ctypes.data_as(_dp)))
+        return e
+
+    def block_energies(self, n_res: int, n_str: int) -> np.ndarray:
+        e = np.empty((int(n_res), int(n_str)))
+        self._check(load_library().exx_get_block_energies(self._h, int(n_res), int(n_str), e.ctypes.data_as(_dp)))
         return e
 
     def destroy(self):

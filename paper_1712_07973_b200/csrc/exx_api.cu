@@ -3,7 +3,9 @@
 // Hot path per same-(j,l) batch (PAPER.md:113-117 kernels 1-3, fused): pass A -> pass B -> pass C -> energy reduce,
 // all enqueued on the plan's stream; the host only schedules.  No CPU fallback exists anywhere in this file:
 // without a usable CUDA device every computing entry point returns EXX_ERR_CUDA.
+#include <algorithm>
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -96,8 +98,16 @@ __global__ void permute_kernel_axes(const double* ks_sym, double* ks_perm, int n
     }
 }
 
+// ks[x] *= scale  (host-supplied periodic Fourier table: fold in the 1/T_tot of the inverse transform)
+__global__ void scale_kernel(double* ks, long long total, double scale) {
+    for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
+         x += static_cast<long long>(gridDim.x) * blockDim.x)
+        ks[x] *= scale;
+}
+
 // e_ij = dV * sum over tiles of the per-CTA partial sums of pass C, fixed order (deterministic).
-__global__ void reduce_energy_kernel(const double* epart, int tiles, const XformDesc* desc, int j, int l, int n_orb, double dV,
+// square (rect = 0): e_mat is [n][n], ld = n, written symmetrically; rect = 1: e_mat is [n_res][n_str], ld = n_str, entry (j,i).
+__global__ void reduce_energy_kernel(const double* epart, int tiles, const XformDesc* desc, int j, int l, int n_orb, int rect, double dV,
                                      double* e_mat) {
     __shared__ double sh[2][256];
     const int t = blockIdx.x;
@@ -115,24 +125,28 @@ __global__ void reduce_energy_kernel(const double* epart, int tiles, const Xform
         if (d.flags & 1) {
             const double e1 = dV * sh[0][0];
             e_mat[static_cast<size_t>(j) * n_orb + d.i] = e1;
-            e_mat[static_cast<size_t>(d.i) * n_orb + j] = e1;
+            if (!rect) e_mat[static_cast<size_t>(d.i) * n_orb + j] = e1;
         }
         if (d.flags & 2) {
             const double e2 = dV * sh[1][0];
             e_mat[static_cast<size_t>(l) * n_orb + d.i] = e2;
-            e_mat[static_cast<size_t>(d.i) * n_orb + l] = e2;
+            if (!rect) e_mat[static_cast<size_t>(d.i) * n_orb + l] = e2;
         }
     }
 }
 
-// E_x = -1/2 sum_{i,j} f_i f_j e_ij over ordered pairs (Eq. 5), fixed-order tree.
-__global__ void exchange_energy_kernel(const double* e_mat, const double* occ, int n_orb, double* ex) {
+// E_x = -1/2 sum_{i,j} f_i f_j e_ij over ordered pairs (Eq. 5), fixed-order tree.  e_mat is
+// [n_rows][n_cols] with row occupations occ_r and column occupations occ_c; the square apply passes the same set twice
+// and scale = -1/2; a rectangular block between two disjoint sets holds each of its pairs once but Eq. 5 counts both
+// orders, so scale = -1.
+__global__ void exchange_energy_kernel(const double* e_mat, const double* occ_r, const double* occ_c, int n_rows, int n_cols, double scale,
+                                       double* ex) {
     __shared__ double sh[1024];
-    const long long total = static_cast<long long>(n_orb) * n_orb;
+    const long long total = static_cast<long long>(n_rows) * n_cols;
     double s = 0.0;
     for (long long x = threadIdx.x; x < total; x += blockDim.x) {
-        const int i = static_cast<int>(x / n_orb), j = static_cast<int>(x % n_orb);
-        s += occ[i] * occ[j] * e_mat[x];
+        const int i = static_cast<int>(x / n_cols), j = static_cast<int>(x % n_cols);
+        s += occ_r[i] * occ_c[j] * e_mat[x];
     }
     sh[threadIdx.x] = s;
     __syncthreads();
@@ -140,7 +154,7 @@ __global__ void exchange_energy_kernel(const double* e_mat, const double* occ, i
         if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
         __syncthreads();
     }
-    if (threadIdx.x == 0) *ex = -0.5 * sh[0];
+    if (threadIdx.x == 0) *ex = scale * sh[0];
 }
 
 }  // namespace
@@ -178,10 +192,15 @@ struct exx_plan {
     size_t stage_elems;
     KernelInfo info_a, info_b, info_c;
     long long launches;
-    int last_n_orb;
+    int device;             // ordinal of the device the plan was created on; every entry point switches to it
+    int last_rows, last_cols;   // shape of the energy matrix the most recent apply left in e_mat (0: none)
+    int last_rect;          // 1: that matrix is a rectangular block [n_res][n_str], 0: the symmetric [n][n] one
+    int custom_kernel;      // periodic BC with a host-supplied Fourier table
     int profiling;
-    std::vector<cudaEvent_t> events;   // 5 per batch when profiling
+    std::vector<cudaEvent_t> events;   // 5 per batch when profiling (pool grown by exx_plan_set_profiling / set_batch)
     size_t events_used;
+    Schedule sched;         // reserved for the largest apply at creation: exx_apply* allocate nothing
+    std::vector<char> copied;   // exx_apply_host: rows of K psi already on their way to the host
     size_t ws_bytes;        // batch workspace (W1 + energy partials)
     size_t fixed_bytes;     // tables, descriptors, pair-energy matrix
     std::string err;
@@ -260,6 +279,22 @@ void bsplit_of(int T, int* R1, int* R2) {
     }
 }
 
+struct DeviceGuard {                                        // makes the plan's device current for the scope of an entry point
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) { cudaGetLastError(); ok = false; }
+    }
+    ~DeviceGuard() {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+#define EXX_ENTER(plan)                                                                       \
+    DeviceGuard guard__((plan)->device);                                                      \
+    if (!guard__.ok) return fail(plan, EXX_ERR_CUDA, "cannot switch to the plan's CUDA device")
+
 void free_workspace(exx_plan* p) {
     if (p->w1) cudaFree(p->w1);
     if (p->epart) cudaFree(p->epart);
@@ -267,17 +302,50 @@ void free_workspace(exx_plan* p) {
     p->epart = nullptr;
 }
 
+// upper bound of the number of batches of any apply of this plan with batches of max_batch transforms
+size_t max_batches(const exx_plan* p, int max_batch) {
+    const size_t n = static_cast<size_t>(p->max_orb), rows = (n + 1) / 2;
+    return rows * ((n + max_batch - 1) / max_batch);
+}
+
+// event pool for per-pass profiling: 5 events per batch of the largest apply
+exx_status grow_event_pool(exx_plan* p) {
+    const size_t need = max_batches(p, p->max_batch) * 5;
+    try {
+        p->events.reserve(need);
+    } catch (const std::bad_alloc&) {
+        return fail(p, EXX_ERR_ALLOC, "out of host memory (event pool)");
+    }
+    while (p->events.size() < need) {
+        cudaEvent_t ev;
+        EXX_CUDA(p, cudaEventCreate(&ev));
+        p->events.push_back(ev);
+    }
+    return EXX_OK;
+}
+
+// The new buffers are allocated BEFORE the old ones are released: a failed request (e.g. an absurd batch size) leaves
+// the plan exactly as it was, with its previous workspace and batch size.
 exx_status alloc_workspace(exx_plan* p, int max_batch) {
-    free_workspace(p);
-    p->max_batch = max_batch;
     const size_t w1_bytes = p->w1_elems_per_xform * sizeof(double2) * static_cast<size_t>(max_batch);
     const size_t ep_bytes = static_cast<size_t>(max_batch) * p->info_c.tiles * 2 * sizeof(double);
-    cudaError_t e = cudaMalloc(&p->w1, w1_bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(p, EXX_ERR_ALLOC, "cudaMalloc(workspace W1) failed"); }
-    e = cudaMalloc(&p->epart, ep_bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(p, EXX_ERR_ALLOC, "cudaMalloc(energy partials) failed"); }
+    double2* w1 = nullptr;
+    double* epart = nullptr;
+    if (cudaMalloc(&w1, w1_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(p, EXX_ERR_ALLOC, "cudaMalloc(workspace W1) failed; the previous workspace is kept");
+    }
+    if (cudaMalloc(&epart, ep_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(w1);
+        return fail(p, EXX_ERR_ALLOC, "cudaMalloc(energy partials) failed; the previous workspace is kept");
+    }
+    free_workspace(p);
+    p->w1 = w1;
+    p->epart = epart;
+    p->max_batch = max_batch;
     p->ws_bytes = w1_bytes + ep_bytes;
-    return EXX_OK;
+    return p->profiling ? grow_event_pool(p) : EXX_OK;
 }
 
 // Transforms per batch: as many as fit a 4 GiB intermediate, at most 128.  Measured on B200: a larger intermediate
@@ -314,9 +382,16 @@ exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
     const int threads = 256;
     if (p->bc == EXX_BC_PERIODIC) {
         const int blocks = static_cast<int>((total + threads - 1) / threads < 4096 ? (total + threads - 1) / threads : 4096);
-        ks_periodic_kernel<<<blocks, threads, 0, p->stream>>>(ks_sym, na, nb, nc, 2.0 * kPi / (p->t[0] * p->h[0]),
-                                                              2.0 * kPi / (p->t[1] * p->h[1]),
-                                                              2.0 * kPi / (p->t[2] * p->h[2]), 1.0 / t_tot);
+        if (kernel_host) {
+            // host-supplied Fourier-space filter on the symmetric index range ("only the filter F of kernel 2 would be
+            // different"): K^(s1,s2,s3), s_a = 0..n_a/2, even in every index; 1/T_tot folded in here
+            EXX_CUDA(p, cudaMemcpyAsync(ks_sym, kernel_host, total * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+            scale_kernel<<<blocks, threads, 0, p->stream>>>(ks_sym, static_cast<long long>(total), 1.0 / t_tot);
+        } else {
+            ks_periodic_kernel<<<blocks, threads, 0, p->stream>>>(ks_sym, na, nb, nc, 2.0 * kPi / (p->t[0] * p->h[0]),
+                                                                  2.0 * kPi / (p->t[1] * p->h[1]),
+                                                                  2.0 * kPi / (p->t[2] * p->h[2]), 1.0 / t_tot);
+        }
         EXX_CUDA(p, cudaGetLastError());
         ++p->launches;
         EXX_CUDA(p, permute());
@@ -355,47 +430,73 @@ exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
     return EXX_OK;
 }
 
+// One application of the pair machinery.  SQUARE: one orbital set on both sides (i <= j triangle, diagonal pairs,
+// symmetric energy matrix).  RECTANGULAR: every pair between a resident set and a disjoint streamed set.
+struct Job {
+    bool square;
+    int n_res, n_str;               // square: both = n_orb
+    const double* psi_res;
+    const double* psi_str;
+    double* kpsi_res;               // nullptr: the resident side receives nothing
+    double* kpsi_str;               // nullptr: the streamed side receives nothing
+    const double* occ_res;          // host; nullptr: all zero (exx_apply_to)
+    const double* occ_str;          // host
+    const unsigned char* mask;      // square only, optional
+    bool zero_res, zero_str;        // overwrite (true) or accumulate into (false) the outputs
+    bool skip_empty_streamed;
+    bool energy;                    // pair energies + E_x contribution
+    double* kpsi_host;              // square host path: finished rows are copied out on the copy stream
+};
+
 // kpsi_host != nullptr (exx_apply_host): K psi_j and K psi_l are final once the last batch of block-row {j,l} has run
 // (later block-rows only stream orbitals i > l), so their device-to-host copies overlap the remaining block-rows.
-exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* occ_host, double* kpsi, double* kpsi_host = nullptr) {
+exx_status run_job_unguarded(exx_plan* p, const Job& job) {
+    if (!p->w1 || !p->epart) return fail(p, EXX_ERR_ALLOC, "the plan has no batch workspace");
     // wait until the previous apply's descriptor upload has left the pinned staging buffers
     EXX_CUDA(p, cudaEventSynchronize(p->upload_done));
-    Schedule sched = build_schedule(n_orb, occ_host, p->max_batch);
+    Schedule& sched = p->sched;
+    if (job.square) build_schedule(sched, job.n_str, job.occ_str, p->max_batch, job.mask);
+    else build_schedule_rect(sched, job.n_res, job.occ_res, job.n_str, job.occ_str, job.skip_empty_streamed, p->max_batch);
     if (sched.xforms.size() > p->desc_cap) return fail(p, EXX_ERR_INTERNAL, "descriptor capacity exceeded");
     if (!sched.xforms.empty()) std::memcpy(p->desc_pinned, sched.xforms.data(), sched.xforms.size() * sizeof(XformDesc));
-    std::memcpy(p->occ_pinned, occ_host, sizeof(double) * n_orb);
+    // occupations on the device: [0, max_orb) the rows of the energy matrix (resident set), [max_orb, 2 max_orb) the columns
+    double* occ_r_pinned = p->occ_pinned;
+    double* occ_c_pinned = p->occ_pinned + p->max_orb;
+    for (int k = 0; k < job.n_res; ++k) occ_r_pinned[k] = job.square ? job.occ_str[k] : (job.occ_res ? job.occ_res[k] : 0.0);
+    for (int k = 0; k < job.n_str; ++k) occ_c_pinned[k] = job.occ_str[k];
     cudaStream_t s = p->stream;
     if (!sched.xforms.empty())
         EXX_CUDA(p, cudaMemcpyAsync(p->desc_dev, p->desc_pinned, sched.xforms.size() * sizeof(XformDesc), cudaMemcpyHostToDevice, s));
-    EXX_CUDA(p, cudaMemcpyAsync(p->occ_dev, p->occ_pinned, sizeof(double) * n_orb, cudaMemcpyHostToDevice, s));
+    EXX_CUDA(p, cudaMemcpyAsync(p->occ_dev, p->occ_pinned, sizeof(double) * 2 * p->max_orb, cudaMemcpyHostToDevice, s));
     EXX_CUDA(p, cudaEventRecord(p->upload_done, s));
-    EXX_CUDA(p, cudaMemsetAsync(kpsi, 0, sizeof(double) * static_cast<size_t>(n_orb) * p->M, s));
-    EXX_CUDA(p, cudaMemsetAsync(p->e_mat, 0, sizeof(double) * static_cast<size_t>(n_orb) * n_orb, s));
+    if (job.kpsi_res && job.zero_res)
+        EXX_CUDA(p, cudaMemsetAsync(job.kpsi_res, 0, sizeof(double) * static_cast<size_t>(job.n_res) * p->M, s));
+    if (job.kpsi_str && job.zero_str && !(job.square && job.zero_res))
+        EXX_CUDA(p, cudaMemsetAsync(job.kpsi_str, 0, sizeof(double) * static_cast<size_t>(job.n_str) * p->M, s));
+    const int e_ld = job.n_str;
+    if (job.energy)
+        EXX_CUDA(p, cudaMemsetAsync(p->e_mat, 0, sizeof(double) * static_cast<size_t>(job.n_res) * job.n_str, s));
 
     ArgsAC ac{};
-    ac.psi = psi; ac.kpsi = kpsi; ac.w1 = p->w1; ac.twc = p->tw[2]; ac.twb = p->twb; ac.epart = p->epart;
+    ac.psi = job.psi_str; ac.psi_r = job.psi_res; ac.kpsi = job.kpsi_str; ac.kpsi_r = job.kpsi_res;
+    ac.w1 = p->w1; ac.twc = p->tw[2]; ac.twb = p->twb; ac.epart = p->epart;
     ac.m_points = p->M; ac.na = p->n[0];
     ArgsB ab{};
     ab.w1 = p->w1; ab.twa = p->tw[0]; ab.ks = p->ks; ab.tc = p->t[2];
     ab.npch = p->t[2] / p->geo.chunk;
 
     p->events_used = 0;
-    if (p->profiling) {
-        const size_t need = sched.batches.size() * 5;
-        while (p->events.size() < need) {
-            cudaEvent_t ev;
-            EXX_CUDA(p, cudaEventCreate(&ev));
-            p->events.push_back(ev);
-        }
-    }
+    const bool prof = p->profiling && sched.batches.size() * 5 <= p->events.size();
     auto mark = [&]() -> cudaError_t {
-        if (!p->profiling) return cudaSuccess;
+        if (!prof) return cudaSuccess;
         return cudaEventRecord(p->events[p->events_used++], s);
     };
-    std::vector<char> copied(kpsi_host ? n_orb : 0, 0);
+    if (job.kpsi_host) std::fill(p->copied.begin(), p->copied.begin() + job.n_str, 0);
     for (const Batch& b : sched.batches) {
         ac.desc = p->desc_dev + b.first;
         ac.j = b.j; ac.l = b.l; ac.fj = b.fj; ac.fl = b.fl; ac.count = b.count;
+        ac.jd = job.square ? b.j : -1;
+        ac.ld = job.square ? b.l : -2;
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_a(p->geo, ac, s, nullptr));
         EXX_CUDA(p, mark());
@@ -403,33 +504,82 @@ exx_status apply_impl(exx_plan* p, int n_orb, const double* psi, const double* o
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
         EXX_CUDA(p, mark());
-        reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_c.tiles, ac.desc, b.j, b.l, n_orb, p->dV, p->e_mat);
-        EXX_CUDA(p, cudaGetLastError());
+        p->launches += 3;
+        if (job.energy) {
+            reduce_energy_kernel<<<b.count, 256, 0, s>>>(p->epart, p->info_c.tiles, ac.desc, b.j, b.l, e_ld, job.square ? 0 : 1, p->dV, p->e_mat);
+            EXX_CUDA(p, cudaGetLastError());
+            ++p->launches;
+        }
         EXX_CUDA(p, mark());
-        p->launches += 4;
         const bool row_ends = (&b == &sched.batches.back()) || ((&b)[1].j != b.j);
-        if (kpsi_host && row_ends) {
+        if (job.kpsi_host && row_ends) {
             const size_t rows = b.l >= 0 ? 2 : 1, off = static_cast<size_t>(b.j) * p->M;
             EXX_CUDA(p, cudaEventRecord(p->row_done, s));
             EXX_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->row_done, 0));
-            EXX_CUDA(p, cudaMemcpyAsync(kpsi_host + off, kpsi + off, rows * p->M * sizeof(double), cudaMemcpyDeviceToHost, p->copy_stream));
-            for (size_t r = 0; r < rows; ++r) copied[b.j + r] = 1;
+            EXX_CUDA(p, cudaMemcpyAsync(job.kpsi_host + off, job.kpsi_res + off, rows * p->M * sizeof(double), cudaMemcpyDeviceToHost, p->copy_stream));
+            for (size_t r = 0; r < rows; ++r) p->copied[b.j + r] = 1;
         }
     }
-    if (kpsi_host) {                                       // rows of block-rows without any pair (all occupations zero)
+    if (job.kpsi_host) {                                   // rows of block-rows without any pair (all occupations zero)
         EXX_CUDA(p, cudaEventRecord(p->row_done, s));
         EXX_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->row_done, 0));
-        for (int r = 0; r < n_orb; ++r)
-            if (!copied[r])
-                EXX_CUDA(p, cudaMemcpyAsync(kpsi_host + static_cast<size_t>(r) * p->M, kpsi + static_cast<size_t>(r) * p->M,
+        for (int r = 0; r < job.n_str; ++r)
+            if (!p->copied[r])
+                EXX_CUDA(p, cudaMemcpyAsync(job.kpsi_host + static_cast<size_t>(r) * p->M, job.kpsi_res + static_cast<size_t>(r) * p->M,
                                             p->M * sizeof(double), cudaMemcpyDeviceToHost, p->copy_stream));
         EXX_CUDA(p, cudaEventRecord(p->copy_done, p->copy_stream));
         EXX_CUDA(p, cudaStreamWaitEvent(s, p->copy_done, 0));
     }
-    exchange_energy_kernel<<<1, 1024, 0, s>>>(p->e_mat, p->occ_dev, n_orb, p->ex_dev);
-    EXX_CUDA(p, cudaGetLastError());
-    ++p->launches;
-    p->last_n_orb = n_orb;
+    if (job.energy) {
+        exchange_energy_kernel<<<1, 1024, 0, s>>>(p->e_mat, p->occ_dev, p->occ_dev + p->max_orb, job.n_res, job.n_str,
+                                                  job.square ? -0.5 : -1.0, p->ex_dev);
+        EXX_CUDA(p, cudaGetLastError());
+        ++p->launches;
+        p->last_rows = job.n_res; p->last_cols = job.n_str; p->last_rect = job.square ? 0 : 1;
+    } else {
+        p->last_rows = p->last_cols = 0;
+    }
+    return EXX_OK;
+}
+
+// No exception crosses the C ABI: the schedule vectors are reserved at plan creation, so nothing in the hot path
+// allocates, and anything that throws all the same is turned into a status code here.
+exx_status run_job(exx_plan* p, const Job& job) {
+    exx_status st;
+    try {
+        st = run_job_unguarded(p, job);
+    } catch (const std::bad_alloc&) {
+        st = fail(p, EXX_ERR_ALLOC, "out of host memory in exx_apply");
+    } catch (...) {
+        st = fail(p, EXX_ERR_INTERNAL, "unexpected exception in exx_apply");
+    }
+    if (st != EXX_OK && job.kpsi_host && p->copy_stream) {
+        // device-to-host copies of finished rows may still be in flight into the caller's buffer
+        cudaStreamSynchronize(p->copy_stream);
+        cudaStreamSynchronize(p->stream);
+        cudaGetLastError();
+    }
+    return st;
+}
+
+bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
+
+bool ranges_overlap(const double* a, size_t na, const double* b, size_t nb) {
+    const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), a1 = a0 + na * sizeof(double);
+    const uintptr_t b0 = reinterpret_cast<uintptr_t>(b), b1 = b0 + nb * sizeof(double);
+    return a0 < b1 && b0 < a1;
+}
+
+// common checks of the device-pointer entry points: psi-like arrays must be 16-byte aligned device memory (the TMA
+// bulk copies and bulk reduce-adds of passes A / C move 16-byte units), outputs must not overlap any input
+exx_status check_set(exx_plan* p, int n, const double* psi, const double* kpsi, const char* what) {
+    if (n < 1 || n > p->max_orb) return fail(p, EXX_ERR_INVALID_ARG, std::string(what) + ": orbital count outside [1, max_orbitals]");
+    if (!psi) return fail(p, EXX_ERR_INVALID_ARG, std::string(what) + ": NULL orbital array");
+    if (!is_device_pointer(psi) || (kpsi && !is_device_pointer(kpsi)))
+        return fail(p, EXX_ERR_BAD_POINTER, std::string(what) + ": orbital arrays must be device pointers");
+    if (!aligned16(psi) || (kpsi && !aligned16(kpsi)))
+        return fail(p, EXX_ERR_INVALID_ARG, std::string(what) + ": orbital arrays must be 16-byte aligned");
+    if ((p->M & 1) != 0) return fail(p, EXX_ERR_INTERNAL, "odd grid size");
     return EXX_OK;
 }
 
@@ -440,12 +590,38 @@ exx_status check_apply_args(exx_plan* p, int n_orb, const void* psi, const doubl
     return EXX_OK;
 }
 
+exx_status square_device_apply(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, const unsigned char* mask,
+                               double* kpsi_dev) {
+    exx_status st = check_set(p, n_orb, psi_dev, kpsi_dev, "exx_apply");
+    if (st != EXX_OK) return st;
+    if (is_device_pointer(occ_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host must be a host pointer");
+    const size_t elems = static_cast<size_t>(n_orb) * p->M;
+    if (ranges_overlap(psi_dev, elems, kpsi_dev, elems)) return fail(p, EXX_ERR_INVALID_ARG, "kpsi must not overlap psi");
+    Job job{};
+    job.square = true;
+    job.n_res = job.n_str = n_orb;
+    job.psi_res = job.psi_str = psi_dev;
+    job.kpsi_res = job.kpsi_str = kpsi_dev;
+    job.occ_res = job.occ_str = occ_host;
+    job.mask = mask;
+    job.zero_res = job.zero_str = true;
+    job.energy = true;
+    return run_job(p, job);
+}
+
+exx_status finish_sync(exx_plan* p, double* ex_host) {
+    EXX_CUDA(p, cudaMemcpyAsync(p->ex_pinned, p->ex_dev, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    *ex_host = *p->ex_pinned;
+    return EXX_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------ C ABI
 extern "C" {
 
-const char* exx_version(void) { return "exx-b200 0.1 (sm_100a)"; }
+const char* exx_version(void) { return "exx-b200 0.2 (sm_100a)"; }
 
 const char* exx_status_string(exx_status s) {
     switch (s) {
@@ -465,7 +641,8 @@ const char* exx_last_error(const exx_plan* plan) { return plan ? plan->err.c_str
 exx_status exx_schedule_pairs(int n_orb, const double* occ_host, long long* n_pairs, long long* n_transforms) {
     if (n_orb < 1 || !occ_host || !n_pairs || !n_transforms) return EXX_ERR_INVALID_ARG;
     try {
-        Schedule s = build_schedule(n_orb, occ_host, 1 << 30);
+        Schedule s;
+        build_schedule(s, n_orb, occ_host, 1 << 30);
         *n_pairs = s.n_pairs;
         *n_transforms = static_cast<long long>(s.xforms.size());
     } catch (const std::bad_alloc&) {
@@ -474,22 +651,67 @@ exx_status exx_schedule_pairs(int n_orb, const double* occ_host, long long* n_pa
     return EXX_OK;
 }
 
+static exx_status list_schedule(const Schedule& s, int* xforms_host, long long capacity, long long* n_transforms) {
+    *n_transforms = static_cast<long long>(s.xforms.size());
+    for (size_t b = 0; b < s.batches.size(); ++b) {
+        const Batch& bt = s.batches[b];
+        for (int t = bt.first; t < bt.first + bt.count && t < capacity; ++t) {
+            int* row = xforms_host + static_cast<size_t>(t) * 5;
+            row[0] = bt.j; row[1] = bt.l; row[2] = s.xforms[t].i; row[3] = s.xforms[t].flags; row[4] = static_cast<int>(b);
+        }
+    }
+    return EXX_OK;
+}
+
 exx_status exx_schedule_list(int n_orb, const double* occ_host, int max_batch, int* xforms_host, long long capacity,
                              long long* n_transforms) {
+    return exx_schedule_list_masked(n_orb, occ_host, nullptr, max_batch, xforms_host, capacity, n_transforms);
+}
+
+exx_status exx_schedule_list_masked(int n_orb, const double* occ_host, const unsigned char* pair_mask_host, int max_batch,
+                                    int* xforms_host, long long capacity, long long* n_transforms) {
     if (n_orb < 1 || !occ_host || !n_transforms || capacity < 0 || (capacity > 0 && !xforms_host)) return EXX_ERR_INVALID_ARG;
     try {
-        Schedule s = build_schedule(n_orb, occ_host, max_batch < 1 ? 1 << 30 : max_batch);
-        *n_transforms = static_cast<long long>(s.xforms.size());
-        for (size_t b = 0; b < s.batches.size(); ++b) {
-            const Batch& bt = s.batches[b];
-            for (int t = bt.first; t < bt.first + bt.count && t < capacity; ++t) {
-                int* row = xforms_host + static_cast<size_t>(t) * 5;
-                row[0] = bt.j; row[1] = bt.l; row[2] = s.xforms[t].i; row[3] = s.xforms[t].flags; row[4] = static_cast<int>(b);
-            }
-        }
+        Schedule s;
+        build_schedule(s, n_orb, occ_host, max_batch < 1 ? 1 << 30 : max_batch, pair_mask_host);
+        return list_schedule(s, xforms_host, capacity, n_transforms);
     } catch (const std::bad_alloc&) {
         return EXX_ERR_ALLOC;
     }
+}
+
+exx_status exx_schedule_list_block(int n_res, const double* occ_res_host, int n_str, const double* occ_str_host, int max_batch,
+                                   int* xforms_host, long long capacity, long long* n_transforms) {
+    if (n_res < 1 || n_str < 1 || !occ_str_host || !n_transforms || capacity < 0 || (capacity > 0 && !xforms_host))
+        return EXX_ERR_INVALID_ARG;
+    try {
+        Schedule s;
+        build_schedule_rect(s, n_res, occ_res_host, n_str, occ_str_host, occ_res_host == nullptr, max_batch < 1 ? 1 << 30 : max_batch);
+        return list_schedule(s, xforms_host, capacity, n_transforms);
+    } catch (const std::bad_alloc&) {
+        return EXX_ERR_ALLOC;
+    }
+}
+
+/* Round-robin exchange of orbital blocks between n_ranks owners (Fig. 1): at step s rank p works on
+ * its own block and the block of rank (p - s) mod P, which it receives from that rank, and sends its own block to
+ * rank (p + s) mod P.  floor(P/2) + 1 steps (s = 0: the diagonal block) cover every unordered block pair exactly once,
+ * except that for even P the last step s = P/2 pairs p with p + P/2 on BOTH ranks: each of the two then takes one half
+ * of the resident rows (what = 2: the rank owning the lower block takes the first half of ITS block as resident rows
+ * against the whole visiting block; what = 3: the other rank takes the visiting block's second half, streamed, against
+ * its whole own block as resident rows). */
+exx_status exx_round_robin_step(int n_ranks, int rank, int step, int* send_to, int* recv_from, int* what) {
+    if (n_ranks < 1 || rank < 0 || rank >= n_ranks || step < 0 || step > n_ranks / 2 || !send_to || !recv_from || !what)
+        return EXX_ERR_INVALID_ARG;
+    if (step == 0) {
+        *send_to = *recv_from = rank;
+        *what = 0;                                         // diagonal block: the square apply of the own orbitals
+        return EXX_OK;
+    }
+    *send_to = (rank + step) % n_ranks;
+    *recv_from = ((rank - step) % n_ranks + n_ranks) % n_ranks;
+    if (n_ranks % 2 == 0 && step == n_ranks / 2) *what = rank < *recv_from ? 2 : 3;
+    else *what = 1;                                        // full rectangular block own x visiting
     return EXX_OK;
 }
 
@@ -500,7 +722,6 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     *plan = nullptr;
     if (bc != EXX_BC_PERIODIC && bc != EXX_BC_FREE) return fail(nullptr, EXX_ERR_INVALID_ARG, "unknown boundary condition");
     if (bc == EXX_BC_FREE && !kernel_host) return fail(nullptr, EXX_ERR_INVALID_ARG, "free BC needs a kernel table");
-    if (bc == EXX_BC_PERIODIC && kernel_host) return fail(nullptr, EXX_ERR_INVALID_ARG, "periodic BC takes no kernel table");
     if (max_orbitals < 1) return fail(nullptr, EXX_ERR_INVALID_ARG, "max_orbitals < 1");
     for (int ax = 0; ax < 3; ++ax) {
         if (dims[ax] < 1) return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE, "non-positive grid length");
@@ -511,10 +732,8 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     geo.ta = geo.free_bc ? 2 * dims[0] : dims[0];
     geo.tb = geo.free_bc ? 2 * dims[1] : dims[1];
     geo.tc = geo.free_bc ? 2 * dims[2] : dims[2];
-    if (!geometry_supported(geo))
-        return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE,
-                    "transform lengths must be in {16,32,64,96,128,192,256}; non-cubic grids only with lengths <= 64");
-    geo.chunk = chunk_for(geo.ta, geo.tb, geo.free_bc != 0);
+    if (!geometry_supported(geo)) return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE, unsupported_geometry_text());
+    geo.chunk = chunk_of(geo);
 
     int ndev = 0;
     cudaError_t ce = cudaGetDeviceCount(&ndev);
@@ -527,6 +746,11 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
 
     exx_plan* p = new (std::nothrow) exx_plan();
     if (!p) return fail(nullptr, EXX_ERR_ALLOC, "out of host memory");
+    if (cudaGetDevice(&p->device) != cudaSuccess || p->device < 0 || p->device >= kMaxDevices) {
+        cudaGetLastError();
+        delete p;
+        return fail(nullptr, EXX_ERR_CUDA, "cannot identify the current CUDA device");
+    }
     p->bc = bc;
     p->geo = geo;
     p->dV = 1.0;
@@ -540,6 +764,7 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     p->t[0] = geo.ta; p->t[1] = geo.tb; p->t[2] = geo.tc;
     p->max_orb = max_orbitals;
     p->stream = static_cast<cudaStream_t>(cuda_stream);
+    p->custom_kernel = (bc == EXX_BC_PERIODIC && kernel_host) ? 1 : 0;
 
     auto bail = [&](exx_status st) {
         g_create_error = p->err;
@@ -549,6 +774,12 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     if (query_pass_a(geo, &p->info_a) != cudaSuccess || query_pass_b(geo, &p->info_b) != cudaSuccess ||
         query_pass_c(geo, &p->info_c) != cudaSuccess)
         return bail(fail(p, EXX_ERR_INTERNAL, "no kernel instantiation for this geometry"));
+    try {
+        reserve_schedule(p->sched, static_cast<size_t>(max_orbitals), static_cast<size_t>(max_orbitals));
+        p->copied.assign(static_cast<size_t>(max_orbitals), 0);
+    } catch (const std::bad_alloc&) {
+        return bail(fail(p, EXX_ERR_ALLOC, "out of host memory (schedule storage)"));
+    }
 
     for (int ax = 0; ax < 3; ++ax) {
         std::vector<double2> tw, roots;
@@ -587,20 +818,24 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     if (st != EXX_OK) return bail(st);
 
     const size_t n = static_cast<size_t>(max_orbitals);
-    p->desc_cap = n * (n + 3) / 4 + n + 4;
+    p->desc_cap = max_transforms(n, n);
     bool ok = cudaMalloc(&p->e_mat, n * n * sizeof(double)) == cudaSuccess &&
-              cudaMalloc(&p->occ_dev, n * sizeof(double)) == cudaSuccess &&
+              cudaMalloc(&p->occ_dev, 2 * n * sizeof(double)) == cudaSuccess &&
               cudaMalloc(&p->desc_dev, p->desc_cap * sizeof(XformDesc)) == cudaSuccess &&
               cudaMalloc(&p->ex_dev, sizeof(double)) == cudaSuccess &&
               cudaMallocHost(&p->desc_pinned, p->desc_cap * sizeof(XformDesc)) == cudaSuccess &&
-              cudaMallocHost(&p->occ_pinned, n * sizeof(double)) == cudaSuccess &&
+              cudaMallocHost(&p->occ_pinned, 2 * n * sizeof(double)) == cudaSuccess &&
               cudaMallocHost(&p->ex_pinned, sizeof(double)) == cudaSuccess &&
-              cudaEventCreateWithFlags(&p->upload_done, cudaEventDisableTiming) == cudaSuccess;
+              cudaEventCreateWithFlags(&p->upload_done, cudaEventDisableTiming) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&p->row_done, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&p->copy_done, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         return bail(fail(p, EXX_ERR_ALLOC, "allocation of plan buffers failed"));
     }
-    p->fixed_bytes = n * n * sizeof(double) + n * sizeof(double) + p->desc_cap * sizeof(XformDesc) +
+    std::memset(p->occ_pinned, 0, 2 * n * sizeof(double));
+    p->fixed_bytes = n * n * sizeof(double) + 2 * n * sizeof(double) + p->desc_cap * sizeof(XformDesc) +
                      sizeof(double) * (static_cast<size_t>(p->t[0] / 2 + 1) * (p->t[1] / 2 + 1) * p->t[2]);
     if (cudaMemset(p->e_mat, 0, n * n * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
@@ -612,7 +847,9 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
 
 exx_status exx_plan_destroy(exx_plan* p) {
     if (!p) return EXX_OK;
+    DeviceGuard guard(p->device);
     if (p->stream || p->w1) cudaStreamSynchronize(p->stream);
+    if (p->copy_stream) cudaStreamSynchronize(p->copy_stream);
     for (int ax = 0; ax < 3; ++ax) {
         if (p->tw[ax]) cudaFree(p->tw[ax]);
     }
@@ -644,9 +881,11 @@ exx_status exx_plan_transform_dims(const exx_plan* p, int tdims[3]) {
     return EXX_OK;
 }
 
-size_t exx_plan_workspace_bytes(const exx_plan* p) { return p ? p->ws_bytes + p->fixed_bytes : 0; }
+size_t exx_plan_workspace_bytes(const exx_plan* p) { return p ? p->ws_bytes + p->fixed_bytes + 2 * p->stage_elems * sizeof(double) : 0; }
 
 long long exx_plan_launch_count(const exx_plan* p) { return p ? p->launches : 0; }
+
+int exx_plan_device(const exx_plan* p) { return p ? p->device : -1; }
 
 const char* exx_plan_kernel_name(const exx_plan* p, int pass) {
     if (!p) return "";
@@ -656,14 +895,20 @@ const char* exx_plan_kernel_name(const exx_plan* p, int pass) {
 
 exx_status exx_plan_set_profiling(exx_plan* p, int enable) {
     if (!p) return EXX_ERR_INVALID_ARG;
+    EXX_ENTER(p);
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
-    p->profiling = enable ? 1 : 0;
     p->events_used = 0;
+    if (enable) {
+        exx_status st = grow_event_pool(p);
+        if (st != EXX_OK) return st;
+    }
+    p->profiling = enable ? 1 : 0;
     return EXX_OK;
 }
 
 exx_status exx_plan_get_profile(exx_plan* p, double pass_ms[4], long long pass_launches[4]) {
     if (!p || !pass_ms || !pass_launches) return EXX_ERR_INVALID_ARG;
+    EXX_ENTER(p);
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
     for (int k = 0; k < 4; ++k) { pass_ms[k] = 0.0; pass_launches[k] = 0; }
     for (size_t b = 0; b + 5 <= p->events_used; b += 5) {
@@ -679,6 +924,7 @@ exx_status exx_plan_get_profile(exx_plan* p, double pass_ms[4], long long pass_l
 
 exx_status exx_plan_set_batch(exx_plan* p, int max_transforms_per_batch) {
     if (!p) return EXX_ERR_INVALID_ARG;
+    EXX_ENTER(p);
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
     int b = max_transforms_per_batch > 0 ? max_transforms_per_batch : default_batch(p);
     if (b > 4096) b = 4096;
@@ -688,11 +934,9 @@ exx_status exx_plan_set_batch(exx_plan* p, int max_transforms_per_batch) {
 exx_status exx_apply_async(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, double* kpsi_dev, double* ex_dev) {
     exx_status st = check_apply_args(p, n_orb, psi_dev, occ_host, kpsi_dev, ex_dev);
     if (st != EXX_OK) return st;
-    if (!is_device_pointer(psi_dev) || !is_device_pointer(kpsi_dev) || !is_device_pointer(ex_dev))
-        return fail(p, EXX_ERR_BAD_POINTER, "psi_dev, kpsi_dev and ex_dev must be device pointers");
-    if (is_device_pointer(occ_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host must be a host pointer");
-    if (psi_dev == kpsi_dev) return fail(p, EXX_ERR_INVALID_ARG, "kpsi must not alias psi");
-    st = apply_impl(p, n_orb, psi_dev, occ_host, kpsi_dev);
+    EXX_ENTER(p);
+    if (!is_device_pointer(ex_dev)) return fail(p, EXX_ERR_BAD_POINTER, "psi_dev, kpsi_dev and ex_dev must be device pointers");
+    st = square_device_apply(p, n_orb, psi_dev, occ_host, nullptr, kpsi_dev);
     if (st != EXX_OK) return st;
     EXX_CUDA(p, cudaMemcpyAsync(ex_dev, p->ex_dev, sizeof(double), cudaMemcpyDeviceToDevice, p->stream));
     return EXX_OK;
@@ -701,55 +945,158 @@ exx_status exx_apply_async(exx_plan* p, int n_orb, const double* psi_dev, const 
 exx_status exx_apply(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, double* kpsi_dev, double* ex_host) {
     exx_status st = check_apply_args(p, n_orb, psi_dev, occ_host, kpsi_dev, ex_host);
     if (st != EXX_OK) return st;
-    if (!is_device_pointer(psi_dev) || !is_device_pointer(kpsi_dev))
-        return fail(p, EXX_ERR_BAD_POINTER, "psi_dev and kpsi_dev must be device pointers");
-    if (is_device_pointer(occ_host) || is_device_pointer(ex_host))
-        return fail(p, EXX_ERR_BAD_POINTER, "occ_host and ex_host must be host pointers");
-    if (psi_dev == kpsi_dev) return fail(p, EXX_ERR_INVALID_ARG, "kpsi must not alias psi");
-    st = apply_impl(p, n_orb, psi_dev, occ_host, kpsi_dev);
+    EXX_ENTER(p);
+    if (is_device_pointer(ex_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host and ex_host must be host pointers");
+    st = square_device_apply(p, n_orb, psi_dev, occ_host, nullptr, kpsi_dev);
     if (st != EXX_OK) return st;
-    EXX_CUDA(p, cudaMemcpyAsync(p->ex_pinned, p->ex_dev, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    return finish_sync(p, ex_host);
+}
+
+exx_status exx_apply_pairs(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, const unsigned char* pair_mask_host,
+                           double* kpsi_dev, double* ex_host) {
+    exx_status st = check_apply_args(p, n_orb, psi_dev, occ_host, kpsi_dev, ex_host);
+    if (st != EXX_OK) return st;
+    EXX_ENTER(p);
+    if (!pair_mask_host) return fail(p, EXX_ERR_INVALID_ARG, "NULL pair mask");
+    if (is_device_pointer(ex_host) || is_device_pointer(pair_mask_host))
+        return fail(p, EXX_ERR_BAD_POINTER, "occ_host, pair_mask_host and ex_host must be host pointers");
+    for (int a = 0; a < n_orb; ++a)
+        for (int b = a + 1; b < n_orb; ++b)
+            if ((pair_mask_host[static_cast<size_t>(a) * n_orb + b] != 0) != (pair_mask_host[static_cast<size_t>(b) * n_orb + a] != 0))
+                return fail(p, EXX_ERR_INVALID_ARG, "the pair mask must be symmetric");
+    st = square_device_apply(p, n_orb, psi_dev, occ_host, pair_mask_host, kpsi_dev);
+    if (st != EXX_OK) return st;
+    return finish_sync(p, ex_host);
+}
+
+exx_status exx_apply_to(exx_plan* p, int n_occ, const double* psi_dev, const double* occ_host, int n_tgt, const double* phi_dev,
+                        double* kphi_dev) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    if (!psi_dev || !occ_host || !phi_dev || !kphi_dev) return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
+    EXX_ENTER(p);
+    exx_status st = check_set(p, n_occ, psi_dev, nullptr, "exx_apply_to (occupied set)");
+    if (st != EXX_OK) return st;
+    st = check_set(p, n_tgt, phi_dev, kphi_dev, "exx_apply_to (target set)");
+    if (st != EXX_OK) return st;
+    if (is_device_pointer(occ_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host must be a host pointer");
+    const size_t e_occ = static_cast<size_t>(n_occ) * p->M, e_tgt = static_cast<size_t>(n_tgt) * p->M;
+    if (ranges_overlap(kphi_dev, e_tgt, psi_dev, e_occ) || ranges_overlap(kphi_dev, e_tgt, phi_dev, e_tgt))
+        return fail(p, EXX_ERR_INVALID_ARG, "kphi must not overlap psi or phi");
+    Job job{};
+    job.square = false;
+    job.n_res = n_tgt; job.n_str = n_occ;
+    job.psi_res = phi_dev; job.psi_str = psi_dev;
+    job.kpsi_res = kphi_dev; job.kpsi_str = nullptr;
+    job.occ_res = nullptr; job.occ_str = occ_host;
+    job.zero_res = true;
+    job.skip_empty_streamed = true;
+    job.energy = false;
+    st = run_job(p, job);
+    if (st != EXX_OK) return st;
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
-    *ex_host = *p->ex_pinned;
     return EXX_OK;
+}
+
+exx_status exx_apply_block(exx_plan* p, int n_res, const double* psi_res_dev, const double* occ_res_host, double* kpsi_res_dev, int n_str,
+                           const double* psi_str_dev, const double* occ_str_host, double* kpsi_str_dev, int flags, double* ex_host) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    if (!psi_res_dev || !occ_res_host || !kpsi_res_dev || !psi_str_dev || !occ_str_host || !kpsi_str_dev || !ex_host)
+        return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
+    if (flags & ~(EXX_BLOCK_ACCUMULATE_RESIDENT | EXX_BLOCK_ACCUMULATE_STREAMED)) return fail(p, EXX_ERR_INVALID_ARG, "unknown flag");
+    EXX_ENTER(p);
+    exx_status st = check_set(p, n_res, psi_res_dev, kpsi_res_dev, "exx_apply_block (resident set)");
+    if (st != EXX_OK) return st;
+    st = check_set(p, n_str, psi_str_dev, kpsi_str_dev, "exx_apply_block (streamed set)");
+    if (st != EXX_OK) return st;
+    if (is_device_pointer(occ_res_host) || is_device_pointer(occ_str_host) || is_device_pointer(ex_host))
+        return fail(p, EXX_ERR_BAD_POINTER, "occupations and ex_host must be host pointers");
+    const size_t e_res = static_cast<size_t>(n_res) * p->M, e_str = static_cast<size_t>(n_str) * p->M;
+    if (ranges_overlap(psi_res_dev, e_res, psi_str_dev, e_str))
+        return fail(p, EXX_ERR_INVALID_ARG, "the two orbital sets must be disjoint (use exx_apply for a set with itself)");
+    if (ranges_overlap(kpsi_res_dev, e_res, kpsi_str_dev, e_str) || ranges_overlap(kpsi_res_dev, e_res, psi_res_dev, e_res) ||
+        ranges_overlap(kpsi_res_dev, e_res, psi_str_dev, e_str) || ranges_overlap(kpsi_str_dev, e_str, psi_res_dev, e_res) ||
+        ranges_overlap(kpsi_str_dev, e_str, psi_str_dev, e_str))
+        return fail(p, EXX_ERR_INVALID_ARG, "outputs must not overlap each other or the inputs");
+    Job job{};
+    job.square = false;
+    job.n_res = n_res; job.n_str = n_str;
+    job.psi_res = psi_res_dev; job.psi_str = psi_str_dev;
+    job.kpsi_res = kpsi_res_dev; job.kpsi_str = kpsi_str_dev;
+    job.occ_res = occ_res_host; job.occ_str = occ_str_host;
+    job.zero_res = !(flags & EXX_BLOCK_ACCUMULATE_RESIDENT);
+    job.zero_str = !(flags & EXX_BLOCK_ACCUMULATE_STREAMED);
+    job.energy = true;
+    st = run_job(p, job);
+    if (st != EXX_OK) return st;
+    return finish_sync(p, ex_host);
 }
 
 exx_status exx_apply_host(exx_plan* p, int n_orb, const double* psi_host, const double* occ_host, double* kpsi_host, double* ex_host) {
     exx_status st = check_apply_args(p, n_orb, psi_host, occ_host, kpsi_host, ex_host);
     if (st != EXX_OK) return st;
+    EXX_ENTER(p);
     if (is_device_pointer(psi_host) || is_device_pointer(kpsi_host) || is_device_pointer(occ_host) || is_device_pointer(ex_host))
         return fail(p, EXX_ERR_BAD_POINTER, "exx_apply_host takes host pointers");
     const size_t elems = static_cast<size_t>(n_orb) * p->M;
+    if (ranges_overlap(psi_host, elems, kpsi_host, elems)) return fail(p, EXX_ERR_INVALID_ARG, "kpsi must not overlap psi");
     if (elems > p->stage_elems) {
+        // grow the staging pair; the old pair is released first (psi + K psi of C5 are 2 x 58 GB: no room for two pairs)
+        EXX_CUDA(p, cudaStreamSynchronize(p->stream));
         if (p->psi_stage) cudaFree(p->psi_stage);
         if (p->kpsi_stage) cudaFree(p->kpsi_stage);
         p->psi_stage = p->kpsi_stage = nullptr;
         p->stage_elems = 0;
         if (cudaMalloc(&p->psi_stage, elems * sizeof(double)) != cudaSuccess || cudaMalloc(&p->kpsi_stage, elems * sizeof(double)) != cudaSuccess) {
             cudaGetLastError();
-            return fail(p, EXX_ERR_ALLOC, "cudaMalloc(host staging) failed");
+            if (p->psi_stage) cudaFree(p->psi_stage);
+            p->psi_stage = p->kpsi_stage = nullptr;
+            return fail(p, EXX_ERR_ALLOC, "cudaMalloc(device staging for exx_apply_host) failed");
         }
         p->stage_elems = elems;
     }
-    if (!p->copy_stream) {
-        EXX_CUDA(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
-        EXX_CUDA(p, cudaEventCreateWithFlags(&p->row_done, cudaEventDisableTiming));
-        EXX_CUDA(p, cudaEventCreateWithFlags(&p->copy_done, cudaEventDisableTiming));
-    }
     EXX_CUDA(p, cudaMemcpyAsync(p->psi_stage, psi_host, elems * sizeof(double), cudaMemcpyHostToDevice, p->stream));
-    st = apply_impl(p, n_orb, p->psi_stage, occ_host, p->kpsi_stage, kpsi_host);
+    Job job{};
+    job.square = true;
+    job.n_res = job.n_str = n_orb;
+    job.psi_res = job.psi_str = p->psi_stage;
+    job.kpsi_res = job.kpsi_str = p->kpsi_stage;
+    job.occ_res = job.occ_str = occ_host;
+    job.zero_res = job.zero_str = true;
+    job.energy = true;
+    job.kpsi_host = kpsi_host;
+    st = run_job(p, job);
     if (st != EXX_OK) return st;
-    EXX_CUDA(p, cudaMemcpyAsync(p->ex_pinned, p->ex_dev, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    return finish_sync(p, ex_host);
+}
+
+exx_status exx_plan_release_staging(exx_plan* p) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    EXX_ENTER(p);
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
-    *ex_host = *p->ex_pinned;
+    if (p->psi_stage) cudaFree(p->psi_stage);
+    if (p->kpsi_stage) cudaFree(p->kpsi_stage);
+    p->psi_stage = p->kpsi_stage = nullptr;
+    p->stage_elems = 0;
     return EXX_OK;
 }
 
-exx_status exx_get_pair_energies(exx_plan* p, double* e_host) {
+exx_status exx_get_pair_energies(exx_plan* p, int n_orb, double* e_host) {
     if (!p || !e_host) return EXX_ERR_INVALID_ARG;
-    if (p->last_n_orb < 1) return fail(p, EXX_ERR_INVALID_ARG, "no apply has run on this plan");
-    const size_t n = static_cast<size_t>(p->last_n_orb);
+    EXX_ENTER(p);
+    if (p->last_rows < 1 || p->last_rect) return fail(p, EXX_ERR_INVALID_ARG, "the most recent apply left no symmetric pair-energy matrix");
+    if (n_orb != p->last_rows) return fail(p, EXX_ERR_INVALID_ARG, "n_orb differs from the orbital count of the most recent apply");
+    const size_t n = static_cast<size_t>(n_orb);
     EXX_CUDA(p, cudaMemcpyAsync(e_host, p->e_mat, n * n * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    return EXX_OK;
+}
+
+exx_status exx_get_block_energies(exx_plan* p, int n_res, int n_str, double* e_host) {
+    if (!p || !e_host) return EXX_ERR_INVALID_ARG;
+    EXX_ENTER(p);
+    if (p->last_rows < 1 || !p->last_rect) return fail(p, EXX_ERR_INVALID_ARG, "the most recent apply was not exx_apply_block");
+    if (n_res != p->last_rows || n_str != p->last_cols) return fail(p, EXX_ERR_INVALID_ARG, "block shape differs from the most recent exx_apply_block");
+    EXX_CUDA(p, cudaMemcpyAsync(e_host, p->e_mat, static_cast<size_t>(n_res) * n_str * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
     EXX_CUDA(p, cudaStreamSynchronize(p->stream));
     return EXX_OK;
 }

@@ -3,6 +3,8 @@
 
 #include <cuda_runtime.h>
 
+#include <mutex>
+
 #include "exx_passes.cuh"
 
 namespace exx {
@@ -27,6 +29,9 @@ bool length_supported(int t);
 // True if kernels for this (ta,tb,tc,bc) combination are compiled in (cubic grids of every supported length;
 // any mix of lengths <= 64).
 bool geometry_supported(const Geometry& g);
+// W1 layout parameter CHUNK of a supported geometry, and the text of the EXX_ERR_UNSUPPORTED_SIZE message.
+int chunk_of(const Geometry& g);
+const char* unsupported_geometry_text();
 
 // Each returns cudaSuccess or the launch/attribute error.  count = transforms in the batch.
 cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info);
@@ -36,6 +41,41 @@ cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, cudaStream_t s,
 cudaError_t query_pass_a(const Geometry& g, KernelInfo* info);
 cudaError_t query_pass_b(const Geometry& g, KernelInfo* info);
 cudaError_t query_pass_c(const Geometry& g, KernelInfo* info);
+
+// Per-kernel, per-device launch state.  cudaFuncSetAttribute(MaxDynamicSharedMemorySize) applies to the CURRENT device
+// only, so the opt-in and the occupancy it yields are cached per device ordinal (plans on different GPUs of one process
+// are independent); the mutex makes the first launches of two host threads safe.
+constexpr int kMaxDevices = 64;
+struct LaunchCache {
+    std::mutex m;
+    int occ[kMaxDevices];
+    int sms[kMaxDevices];
+    LaunchCache() { for (int d = 0; d < kMaxDevices; ++d) { occ[d] = -1; sms[d] = 0; } }
+};
+// Makes `kern` launchable with `smem` bytes of dynamic shared memory on the current device; reports the resident CTAs
+// per SM for `nt` threads and the device's SM count.
+template <class K>
+inline cudaError_t prepare_launch(K kern, int smem, int nt, LaunchCache& c, int* ctas_per_sm, int* sm_count = nullptr) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(c.m);
+    if (c.occ[dev] < 0) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        int occ = 0, sms = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nt, smem);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        c.sms[dev] = sms > 0 ? sms : 148;
+        c.occ[dev] = occ;
+    }
+    *ctas_per_sm = c.occ[dev];
+    if (sm_count) *sm_count = c.sms[dev];
+    return cudaSuccess;
+}
 
 // Compile-time tuning shared by the instantiation files -------------------------------------------------------
 constexpr int kSmemPerSM = 227 * 1024;                     // usable shared memory per SM (and per CTA, opt-in)

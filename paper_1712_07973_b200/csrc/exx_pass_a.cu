@@ -4,18 +4,6 @@
 
 namespace exx {
 
-template <class K>
-static cudaError_t prepare(K kern, int smem, int nt, bool* done, int* ctas_per_sm) {
-    if (!*done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, nt, smem);
-        if (e != cudaSuccess) return e;
-        *done = true;
-    }
-    return cudaSuccess;
-}
-
 template <int TC, int TB, bool FREE>
 static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
     using T = TuneAC<TC, TB, FREE>;
@@ -25,11 +13,11 @@ static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     constexpr int smem = ws ? T::SMEM_A_WS : T::SMEM_A;
     constexpr int nt = ws ? 32 * (T::NAW + T::NBW) : T::NT_A;
     auto kern = ws ? pass_a_ws_kernel<C, T::NAW, T::NBW, T::NSTG_A_WS, T::MINB_A_WS> : pass_a_kernel<C, T::NT_A, T::NSTG_A, T::MINB_A>;
-    static bool done = false;
-    static int occ = 0;
-    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; info->name = ws ? "pass_a_ws_kernel" : "pass_a_kernel"; }
+    static LaunchCache cache;
+    int occ = 0;
+    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = 0; info->name = ws ? "pass_a_ws_kernel" : "pass_a_kernel"; }
     if (!launch) return cudaSuccess;
-    cudaError_t e = prepare(kern, smem, nt, &done, &occ);
+    cudaError_t e = prepare_launch(kern, smem, nt, cache, &occ);
     if (e != cudaSuccess) return e;
     if (info) info->ctas_per_sm = occ;
     kern<<<args.na * C::TILES_PER_A, nt, smem, s>>>(args);

@@ -4,30 +4,6 @@
 
 namespace exx {
 
-template <class K>
-static cudaError_t prepare(K kern, int smem, int nt, bool* done, int* ctas_per_sm) {
-    if (!*done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, nt, smem);
-        if (e != cudaSuccess) return e;
-        *done = true;
-    }
-    return cudaSuccess;
-}
-
-static int sm_count() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
-            cudaGetLastError();
-            n = 148;
-        }
-    }
-    return n;
-}
-
 template <int TA, int TB, bool FREE, int CHUNK>
 static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, KernelInfo* info, bool launch) {
     using T = TuneB<TA, TB, FREE, CHUNK>;
@@ -37,17 +13,17 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
     } else {
         auto kern = T::WS ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB, false>
                   : T::WSF ? pass_b_ws_kernel<C, T::NY, T::NX, T::MINB, true> : pass_b_kernel<C, T::NT, T::MINB>;
-        static bool done = false;
-        static int occ = 0;
-        if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = occ; info->name = (T::WS || T::WSF) ? "pass_b_ws_kernel" : "pass_b_kernel"; }
+        static LaunchCache cache;
+        int occ = 0, sms = 148;
+        if (info) { info->threads = T::NT; info->smem_bytes = T::SMEM; info->tiles = C::R1 * args_in.npch; info->ctas_per_sm = 0; info->name = (T::WS || T::WSF) ? "pass_b_ws_kernel" : "pass_b_kernel"; }
         if (!launch) return cudaSuccess;
-        cudaError_t e = prepare(kern, T::SMEM, T::NT, &done, &occ);
+        cudaError_t e = prepare_launch(kern, T::SMEM, T::NT, cache, &occ, &sms);
         if (e != cudaSuccess) return e;
         if (info) info->ctas_per_sm = occ;
         ArgsB args = args_in;
         args.count = count;
         args.ntiles = count * C::R1 * args.npch;
-        const int slots = sm_count() * (occ > 0 ? occ : 1);
+        const int slots = sms * (occ > 0 ? occ : 1);
         const int grid = args.ntiles < slots ? args.ntiles : slots;
         kern<<<grid, T::NT, T::SMEM, s>>>(args);
         return cudaGetLastError();
@@ -77,6 +53,12 @@ cudaError_t query_pass_b(const Geometry& g, KernelInfo* info) {
 
 bool length_supported(int t) {
     return t == 16 || t == 32 || t == 64 || t == 96 || t == 128 || t == 192 || t == 256;
+}
+
+int chunk_of(const Geometry& g) { return chunk_for(g.ta, g.tb, g.free_bc != 0); }
+
+const char* unsupported_geometry_text() {
+    return "transform lengths must be in {16,32,64,96,128,192,256}; non-cubic grids only with lengths <= 64";
 }
 
 bool geometry_supported(const Geometry& g) {

@@ -4,18 +4,6 @@
 
 namespace exx {
 
-template <class K>
-static cudaError_t prepare(K kern, int smem, int nt, bool* done, int* ctas_per_sm) {
-    if (!*done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kern, nt, smem);
-        if (e != cudaSuccess) return e;
-        *done = true;
-    }
-    return cudaSuccess;
-}
-
 template <int TC, int TB, bool FREE>
 static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
     using T = TuneAC<TC, TB, FREE>;
@@ -26,11 +14,11 @@ static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     constexpr bool ws = T::WS_C;
     constexpr int nt = ws ? 32 * (T::NAW_C + T::NBW_C) : T::NT_C;
     auto kern = ws ? pass_c_ws_kernel<C, T::NAW_C, T::NBW_C, 2, T::MINB_C_WS> : pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C>;
-    static bool done = false;
-    static int occ = 0;
-    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = occ; info->name = ws ? "pass_c_ws_kernel" : "pass_c_kernel"; }
+    static LaunchCache cache;
+    int occ = 0;
+    if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = 0; info->name = ws ? "pass_c_ws_kernel" : "pass_c_kernel"; }
     if (!launch) return cudaSuccess;
-    cudaError_t e = prepare(kern, smem, nt, &done, &occ);
+    cudaError_t e = prepare_launch(kern, smem, nt, cache, &occ);
     if (e != cudaSuccess) return e;
     if (info) info->ctas_per_sm = occ;
     kern<<<args.na * C::TILES_PER_A, nt, smem, s>>>(args);

@@ -144,8 +144,10 @@ struct CfgAC {
 };
 
 struct ArgsAC {
-    const double* psi;          // [N][na][nb][nc]
-    double* kpsi;               // pass C only
+    const double* psi;          // streamed set [N][na][nb][nc]: the orbitals i of the transform descriptors
+    const double* psi_r;        // resident set: the orbitals j, l of the batch (== psi for the square apply)
+    double* kpsi;               // pass C: K psi of the streamed set (reduce-add target); nullptr: no streamed update
+    double* kpsi_r;             // pass C: K psi of the resident set (read-modify-write); nullptr: no resident update
     double2* w1;
     const XformDesc* desc;      // first transform of this batch
     const double2* twc;         // [k1*QC + n2] = W_TC^{n2 k1}
@@ -154,6 +156,8 @@ struct ArgsAC {
     long long m_points;         // na*nb*nc
     int na;
     int j, l;                   // resident orbitals of the batch (l < 0: none; the imaginary slot is then never present)
+    int jd, ld;                 // j, l in the numbering of the STREAMED set (square apply: jd = j, ld = l), or negative
+                                // values when the two sets are distinct (rectangular pair block: no diagonal pair exists)
     double fj, fl;
     int count;                  // transforms in the batch
 };
@@ -635,8 +639,9 @@ __host__ __device__ constexpr int ceil_div(int a, int b) { return (a + b - 1) / 
 // TMA bulk loads of the LINES lines of orbital `orb` of tile (a, b2base) into [line][LS] shared memory; the caller has
 // armed `bar` with the byte count (all 32 lanes of one warp call this)
 template <class C>
-__device__ __forceinline__ void issue_line_loads(const ArgsAC& g, int orb, double* dst, uint64_t* bar, int a, int b2base, int lane) {
-    const double* base = g.psi + static_cast<size_t>(orb) * g.m_points;
+__device__ __forceinline__ void issue_line_loads(const ArgsAC& g, const double* set, int orb, double* dst, uint64_t* bar, int a, int b2base,
+                                                 int lane) {
+    const double* base = set + static_cast<size_t>(orb) * g.m_points;
     for (int l = lane; l < C::LINES; l += 32) bulk_g2s(dst + l * C::LS, base + line_offset<C>(l, a, b2base), C::LINE_BYTES, bar);
 }
 // the streamed psi_i lines of one transform into an operand stage
@@ -645,7 +650,7 @@ __device__ __forceinline__ void issue_operand_loads(const ArgsAC& g, const Xform
                                                     int b2base, int lane) {
     if (lane == 0) mbar_arrive_expect_tx(bar, C::LINES * C::LINE_BYTES);
     __syncwarp();
-    issue_line_loads<C>(g, d.i, stage, bar, a, b2base, lane);
+    issue_line_loads<C>(g, g.psi, d.i, stage, bar, a, b2base, lane);
 }
 
 // Pass A.  One CTA per (a, b2-group) tile, looping over the transforms of the same-(j,l) batch.  psi_j and psi_l of the
@@ -679,8 +684,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     for (int m = 0; m < NI0; ++m) {
         const int w = tid + m * NT;
         q0[m] = lineq_index<C, false>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
-        const double* pj = g.psi + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
-        const double* pl = g.psi + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
+        const double* pj = g.psi_r + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
+        const double* pl = g.psi_r + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
 #pragma unroll
         for (int n1 = 0; n1 < C::PCN; ++n1) { vj[m][n1] = ld_ro(pj + C::QC * n1); vl[m][n1] = ld_ro(pl + C::QC * n1); }
     }
@@ -756,8 +761,8 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_a_ws_kernel(const
         for (int m = 0; m < NI0; ++m) {
             const int w = tid + m * AT;
             q0[m] = lineq_index<C, false>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
-            const double* pj = g.psi + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
-            const double* pl = g.psi + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
+            const double* pj = g.psi_r + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
+            const double* pl = g.psi_r + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
 #pragma unroll
             for (int n1 = 0; n1 < C::PCN; ++n1) { vj[m][n1] = ld_ro(pj + C::QC * n1); vl[m][n1] = ld_ro(pl + C::QC * n1); }
         }
@@ -1097,8 +1102,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     if (tid < 32) {
         if (tid == 0) mbar_arrive_expect_tx(&resbar, 2 * C::LINES * C::LINE_BYTES);
         __syncwarp();
-        issue_line_loads<C>(g, g.j, RES, &resbar, a, b2base, tid);
-        issue_line_loads<C>(g, g.l >= 0 ? g.l : g.j, RES + C::LINES * C::LS, &resbar, a, b2base, tid);
+        issue_line_loads<C>(g, g.psi_r, g.j, RES, &resbar, a, b2base, tid);
+        issue_line_loads<C>(g, g.psi_r, g.l >= 0 ? g.l : g.j, RES + C::LINES * C::LS, &resbar, a, b2base, tid);
         for (int t = 0; t < NSTG && t < g.count; ++t)
             issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
     }
@@ -1146,7 +1151,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
 #pragma unroll
         for (int m = 0; m < NI2; ++m)
             if (tid + m * NT < C::ITEMS_LINE_Q)
-                c2_compute<C>(S + q2[m].row, d, g.l, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                c2_compute<C>(S + q2[m].row, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
                               accj[m], accl[m], e1, e2);
         fence_proxy_async();                               // increments visible to the TMA reads below
         // block reduction of the energy partials in a fixed order (deterministic)
@@ -1166,7 +1171,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         }
         if (tid < 32) {
             // K psi_i += -(f_j V_ji psi_j + f_l V_li psi_l)   (the same V serves both orbitals of a pair)
-            if (d.flags != 0 && d.i != g.j && d.i != g.l) {
+            if (g.kpsi != nullptr && d.flags != 0 && d.i != g.jd && d.i != g.ld) {
                 double* ki = g.kpsi + static_cast<size_t>(d.i) * g.m_points;
                 for (int l = tid; l < C::LINES; l += 32)
                     bulk_red_add_f64(ki + line_offset<C>(l, a, b2base), stage + l * C::LS, C::LINE_BYTES);
@@ -1182,12 +1187,12 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     // K psi_j -= accj, K psi_l -= accl (this CTA is the only writer of its tile of K psi_j, K psi_l in this launch)
 #pragma unroll
     for (int m = 0; m < NI2; ++m)
-        if (tid + m * NT < C::ITEMS_LINE_Q) {
-            double* kj = g.kpsi + static_cast<size_t>(g.j) * g.m_points + q2[m].gofs;
+        if (g.kpsi_r != nullptr && tid + m * NT < C::ITEMS_LINE_Q) {
+            double* kj = g.kpsi_r + static_cast<size_t>(g.j) * g.m_points + q2[m].gofs;
 #pragma unroll
             for (int n1 = 0; n1 < C::PCN; ++n1) kj[C::QC * n1] -= accj[m][n1];
             if (g.l >= 0) {
-                double* kl = g.kpsi + static_cast<size_t>(g.l) * g.m_points + q2[m].gofs;
+                double* kl = g.kpsi_r + static_cast<size_t>(g.l) * g.m_points + q2[m].gofs;
 #pragma unroll
                 for (int n1 = 0; n1 < C::PCN; ++n1) kl[C::QC * n1] -= accl[m][n1];
             }
@@ -1257,8 +1262,8 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_c_ws_kernel(const
         if (tid < 32) {
             if (tid == 0) mbar_arrive_expect_tx(&resbar, 2 * C::LINES * C::LINE_BYTES);
             __syncwarp();
-            issue_line_loads<C>(g, g.j, RES, &resbar, a, b2base, tid);
-            issue_line_loads<C>(g, g.l >= 0 ? g.l : g.j, RES + C::LINES * C::LS, &resbar, a, b2base, tid);
+            issue_line_loads<C>(g, g.psi_r, g.j, RES, &resbar, a, b2base, tid);
+            issue_line_loads<C>(g, g.psi_r, g.l >= 0 ? g.l : g.j, RES + C::LINES * C::LS, &resbar, a, b2base, tid);
             for (int t = 0; t < NSTG && t < g.count; ++t)
                 issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
         }
@@ -1292,7 +1297,7 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_c_ws_kernel(const
 #pragma unroll
             for (int m = 0; m < NI2; ++m)
                 if (tid + m * BT < C::ITEMS_LINE_Q)
-                    c2_compute<C>(S + q2[m].row, d, g.l, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                    c2_compute<C>(S + q2[m].row, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
                                   accj[m], accl[m], e1, e2);
             fence_proxy_async();
 #pragma unroll
@@ -1313,7 +1318,7 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_c_ws_kernel(const
                 ep[0] = s1; ep[1] = s2;
             }
             if (tid < 32) {
-                if (d.flags != 0 && d.i != g.j && d.i != g.l) {
+                if (g.kpsi != nullptr && d.flags != 0 && d.i != g.jd && d.i != g.ld) {
                     double* ki = g.kpsi + static_cast<size_t>(d.i) * g.m_points;
                     for (int l = tid; l < C::LINES; l += 32)
                         bulk_red_add_f64(ki + line_offset<C>(l, a, b2base), stage + l * C::LS, C::LINE_BYTES);
@@ -1329,12 +1334,12 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_c_ws_kernel(const
         }
 #pragma unroll
         for (int m = 0; m < NI2; ++m)
-            if (tid + m * BT < C::ITEMS_LINE_Q) {
-                double* kj = g.kpsi + static_cast<size_t>(g.j) * g.m_points + q2[m].gofs;
+            if (g.kpsi_r != nullptr && tid + m * BT < C::ITEMS_LINE_Q) {
+                double* kj = g.kpsi_r + static_cast<size_t>(g.j) * g.m_points + q2[m].gofs;
 #pragma unroll
                 for (int n1 = 0; n1 < C::PCN; ++n1) kj[C::QC * n1] -= accj[m][n1];
                 if (g.l >= 0) {
-                    double* kl = g.kpsi + static_cast<size_t>(g.l) * g.m_points + q2[m].gofs;
+                    double* kl = g.kpsi_r + static_cast<size_t>(g.l) * g.m_points + q2[m].gofs;
 #pragma unroll
                     for (int n1 = 0; n1 < C::PCN; ++n1) kl[C::QC * n1] -= accl[m][n1];
                 }
