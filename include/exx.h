@@ -214,6 +214,16 @@ exx_status exx_plan_get_profile(exx_plan *plan, double pass_ms[4], long long pas
 /* Tuning knob: maximum packed transforms per batch (same-i group); <= 0 restores the default. */
 exx_status exx_plan_set_batch(exx_plan *plan, int max_transforms_per_batch);
 
+/*
+ * exx_diag_fp64 -- device microbenchmarks for the FP64 leg of the roofline (north_star: "the slower of FFT+fusion bytes
+ * over 8 TB/s HBM and FP64 flops at peak"; MEASURED_PEAKS.json holds no FP64 figure).  Runs on the current device, on
+ * cuda_stream (NULL = default), about 50 ms: dependent-chain DFMA (TFLOP/s, 2 flops per FMA), DADD (1e12 instructions/s:
+ * FFT butterflies are add-heavy, so this is the ceiling in "useful" flops), conflict-free 16-byte shared-memory loads
+ * (GB/s summed over the SMs), and how far the FP64 and shared-memory pipes of an SM overlap when different warps use
+ * them (1 = fully, 0 = serialised).  Diagnostic only: never called by the apply entry points.  Synchronises.
+ */
+exx_status exx_diag_fp64(void *cuda_stream, double *dfma_tflops, double *dadd_tops, double *lds_gbs, double *overlap_ratio);
+
 exx_status  exx_plan_destroy(exx_plan *plan);       /* NULL is allowed */
 const char *exx_status_string(exx_status s);
 const char *exx_last_error(const exx_plan *plan);   /* detail text incl. CUDA error name; plan may be NULL for

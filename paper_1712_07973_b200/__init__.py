@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     ExxError,
     ExxPlan,
     exx_apply,
+    exx_diag_fp64,
     exx_plan_create,
     exx_plan_destroy,
     exx_round_robin_step,

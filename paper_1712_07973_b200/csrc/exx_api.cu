@@ -233,17 +233,7 @@ bool is_device_pointer(const void* p) {
 
 // [k1*Q + n2] = W_T^{n2 k1};  roots[m] = W_T^m.  long double trigonometry, rounded once (no recurrences).
 void host_tables(int T, std::vector<double2>& tw, std::vector<double2>& roots) {
-    int P = 0, Q = 0;
-    switch (T) {
-        case 16: P = Split<16>::P; Q = Split<16>::Q; break;
-        case 32: P = Split<32>::P; Q = Split<32>::Q; break;
-        case 64: P = Split<64>::P; Q = Split<64>::Q; break;
-        case 96: P = Split<96>::P; Q = Split<96>::Q; break;
-        case 128: P = Split<128>::P; Q = Split<128>::Q; break;
-        case 192: P = Split<192>::P; Q = Split<192>::Q; break;
-        case 256: P = Split<256>::P; Q = Split<256>::Q; break;
-        default: break;
-    }
+    const int P = split_p(T), Q = split_q(T);
     const long double two_pi = 6.283185307179586476925286766559005768L;
     roots.resize(T);
     for (int m = 0; m < T; ++m) {
@@ -255,29 +245,9 @@ void host_tables(int T, std::vector<double2>& tw, std::vector<double2>& roots) {
         for (int n2 = 0; n2 < Q; ++n2) tw[k1 * Q + n2] = roots[(k1 * n2) % T];
 }
 
-void split_of(int T, int* P, int* Q) {
-    switch (T) {
-        case 16: *P = Split<16>::P; *Q = Split<16>::Q; break;
-        case 32: *P = Split<32>::P; *Q = Split<32>::Q; break;
-        case 64: *P = Split<64>::P; *Q = Split<64>::Q; break;
-        case 96: *P = Split<96>::P; *Q = Split<96>::Q; break;
-        case 128: *P = Split<128>::P; *Q = Split<128>::Q; break;
-        case 192: *P = Split<192>::P; *Q = Split<192>::Q; break;
-        default: *P = Split<256>::P; *Q = Split<256>::Q; break;
-    }
-}
+void split_of(int T, int* P, int* Q) { *P = split_p(T); *Q = split_q(T); }
 
-void bsplit_of(int T, int* R1, int* R2) {
-    switch (T) {
-        case 16: *R1 = BSplit<16>::R1; *R2 = BSplit<16>::R2; break;
-        case 32: *R1 = BSplit<32>::R1; *R2 = BSplit<32>::R2; break;
-        case 64: *R1 = BSplit<64>::R1; *R2 = BSplit<64>::R2; break;
-        case 96: *R1 = BSplit<96>::R1; *R2 = BSplit<96>::R2; break;
-        case 128: *R1 = BSplit<128>::R1; *R2 = BSplit<128>::R2; break;
-        case 192: *R1 = BSplit<192>::R1; *R2 = BSplit<192>::R2; break;
-        default: *R1 = BSplit<256>::R1; *R2 = BSplit<256>::R2; break;
-    }
-}
+void bsplit_of(int T, int* R1, int* R2) { *R1 = r1_of(T); *R2 = r2_of(T); }
 
 struct DeviceGuard {                                        // makes the plan's device current for the scope of an entry point
     int prev = -1;

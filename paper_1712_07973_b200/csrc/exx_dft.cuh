@@ -193,6 +193,9 @@ struct DftPQ_OP {
     }
 };
 
+template <> struct Dft<6>    { EXX_HD static void run(double* r, double* i) { DftPQ<6, 2, 3, Dft>::run(r, i); } };
+template <> struct DftIP<6>  { EXX_HD static void run(double* r, double* i) { DftPQ<6, 2, 3, DftIP>::run(r, i); } };
+template <> struct DftOP<6>  { EXX_HD static void run(double* r, double* i) { DftPQ_OP<6, 2, 3>::run(r, i); } };
 template <> struct Dft<8>    { EXX_HD static void run(double* r, double* i) { DftPQ<8, 4, 2, Dft>::run(r, i); } };
 template <> struct Dft<12>   { EXX_HD static void run(double* r, double* i) { DftPQ<12, 4, 3, Dft>::run(r, i); } };
 template <> struct Dft<16>   { EXX_HD static void run(double* r, double* i) { DftPQ<16, 4, 4, Dft>::run(r, i); } };

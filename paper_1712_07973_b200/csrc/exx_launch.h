@@ -26,8 +26,8 @@ struct KernelInfo {     // what a launcher reports about the instantiation it di
 
 // Transform lengths the FFT covers.
 bool length_supported(int t);
-// True if kernels for this (ta,tb,tc,bc) combination are compiled in (cubic grids of every supported length;
-// any mix of lengths <= 64).
+// True if kernels for this (ta,tb,tc,bc) combination are compiled in: every mix of the main lengths
+// {16,32,48,64,96,128,144,192,256}, cubic transform grids of the extra lengths {24,72}.
 bool geometry_supported(const Geometry& g);
 // W1 layout parameter CHUNK of a supported geometry, and the text of the EXX_ERR_UNSUPPORTED_SIZE message.
 int chunk_of(const Geometry& g);
@@ -133,9 +133,9 @@ constexpr int pick_line_warps(int items, int cap) {
     return best;
 }
 
-template <int TC, int TB, bool FREE>
+template <int TC, int TB, bool FREE, int CHUNK_>
 struct TuneAC {
-    static constexpr int CHUNK = chunk_for(TC, TB, FREE);
+    static constexpr int CHUNK = CHUNK_;
     // ---- pass C
     static constexpr int G_C = pick_g<TC, TB, FREE>(true, kMaxSmemAC / 2);
     using CfgC = CfgAC<TC, TB, FREE, G_C, CHUNK>;

@@ -1,12 +1,17 @@
-// exx_pass_a.cu -- instantiation + dispatch of pass A (co-density, padding, c-axis FFT, first b-axis stage).
+// exx_pass_a.cu -- instantiation + dispatch of pass A (co-density, padding, c-axis FFT, first b-axis stage) for ONE
+// middle-axis length: compiled once per length with -DEXX_TB=<length> (see exx_inst.cuh).
 #include "exx_inst.cuh"
 #include "exx_launch.h"
 
+#ifndef EXX_TB
+#error "compile with -DEXX_TB=<middle-axis transform length>"
+#endif
+
 namespace exx {
 
-template <int TC, int TB, bool FREE>
-static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
-    using T = TuneAC<TC, TB, FREE>;
+template <int TC, int TB, bool FREE, int CHUNK>
+static cudaError_t run_a_chunk(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+    using T = TuneAC<TC, TB, FREE, CHUNK>;
     using C = typename T::CfgA;
     static_assert(T::SMEM_A == C::SMEM_A * 16 + T::NSTG_A * C::OP_DOUBLES * 8, "pass A shared memory");
     constexpr bool ws = T::WS_A;
@@ -24,23 +29,29 @@ static cudaError_t run_a(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     return cudaGetLastError();
 }
 
-static cudaError_t dispatch_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
-#define X(TC_, TB_)                                                                                  \
-    if (g.tc == TC_ && g.tb == TB_)                                                                  \
-        return g.free_bc ? run_a<TC_, TB_, true>(args, s, info, launch) : run_a<TC_, TB_, false>(args, s, info, launch);
-    EXX_FOR_EACH_PAIR(X)
-#undef X
+template <int TC, int TB, bool FREE>
+static cudaError_t run_a(int chunk, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+    if constexpr (chunk_possible<TB, FREE, 4>()) { if (chunk == 4) return run_a_chunk<TC, TB, FREE, 4>(args, s, info, launch); }
+    if constexpr (chunk_possible<TB, FREE, 2>()) { if (chunk == 2) return run_a_chunk<TC, TB, FREE, 2>(args, s, info, launch); }
+    if constexpr (chunk_possible<TB, FREE, 1>()) { if (chunk == 1) return run_a_chunk<TC, TB, FREE, 1>(args, s, info, launch); }
     return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
-    return dispatch_a(g, args, s, info, true);
-}
-
-cudaError_t query_pass_a(const Geometry& g, KernelInfo* info) {
-    ArgsAC args{};
-    args.na = g.free_bc ? g.ta / 2 : g.ta;
-    return dispatch_a(g, args, nullptr, info, false);
+// true if this translation unit owns the geometry (g.tb == EXX_TB and a compiled g.tc); *err then holds the outcome
+bool EXX_CAT(try_pass_a_, EXX_TB)(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch, cudaError_t* err) {
+    if (g.tb != EXX_TB) return false;
+#define X(TC_)                                                                                                       \
+    if (g.tc == TC_) {                                                                                               \
+        *err = g.free_bc ? run_a<TC_, EXX_TB, true>(g.chunk, args, s, info, launch) : run_a<TC_, EXX_TB, false>(g.chunk, args, s, info, launch); \
+        return true;                                                                                                 \
+    }
+    if constexpr (is_main_length(EXX_TB)) {
+        EXX_MAIN_LENGTHS(X)
+    } else {
+        X(EXX_TB)
+    }
+#undef X
+    return false;
 }
 
 }  // namespace exx

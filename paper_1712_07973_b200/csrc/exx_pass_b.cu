@@ -1,11 +1,17 @@
-// exx_pass_b.cu -- instantiation + dispatch of pass B (second b stage, a-axis FFT, K^ multiply, inverse).
+// exx_pass_b.cu -- instantiation + dispatch of pass B (second b stage, a-axis FFT, K^ multiply, inverse) for ONE
+// middle-axis length: compiled once per length with -DEXX_TB=<length> (see exx_inst.cuh).
 #include "exx_inst.cuh"
 #include "exx_launch.h"
 
+#ifndef EXX_TB
+#error "compile with -DEXX_TB=<middle-axis transform length>"
+#endif
+
 namespace exx {
 
-template <int TA, int TB, bool FREE, int CHUNK>
+template <int TA, int TB, bool FREE>
 static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, KernelInfo* info, bool launch) {
+    constexpr int CHUNK = ChunkOf<TA, TB, FREE>::value;
     using T = TuneB<TA, TB, FREE, CHUNK>;
     using C = typename T::Cfg;
     if constexpr (!T::FITS) {
@@ -30,41 +36,20 @@ static cudaError_t run_b(const ArgsB& args_in, int count, cudaStream_t s, Kernel
     }
 }
 
-static cudaError_t dispatch_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info, bool launch) {
-#define X(TA_, TB_)                                                                                              \
-    if (g.ta == TA_ && g.tb == TB_) {                                                                            \
-        if (g.free_bc) return run_b<TA_, TB_, true, chunk_for(TA_, TB_, true)>(args, count, s, info, launch);     \
-        return run_b<TA_, TB_, false, chunk_for(TA_, TB_, false)>(args, count, s, info, launch);                  \
+bool EXX_CAT(try_pass_b_, EXX_TB)(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info, bool launch, cudaError_t* err) {
+    if (g.tb != EXX_TB) return false;
+#define X(TA_)                                                                                                       \
+    if (g.ta == TA_) {                                                                                               \
+        *err = g.free_bc ? run_b<TA_, EXX_TB, true>(args, count, s, info, launch) : run_b<TA_, EXX_TB, false>(args, count, s, info, launch); \
+        return true;                                                                                                 \
     }
-    EXX_FOR_EACH_PAIR(X)
+    if constexpr (is_main_length(EXX_TB)) {
+        EXX_MAIN_LENGTHS(X)
+    } else {
+        X(EXX_TB)
+    }
 #undef X
-    return cudaErrorInvalidValue;
-}
-
-cudaError_t launch_pass_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info) {
-    return dispatch_b(g, args, count, s, info, true);
-}
-
-cudaError_t query_pass_b(const Geometry& g, KernelInfo* info) {
-    ArgsB args{};
-    args.npch = g.tc / g.chunk;
-    return dispatch_b(g, args, 0, nullptr, info, false);
-}
-
-bool length_supported(int t) {
-    return t == 16 || t == 32 || t == 64 || t == 96 || t == 128 || t == 192 || t == 256;
-}
-
-int chunk_of(const Geometry& g) { return chunk_for(g.ta, g.tb, g.free_bc != 0); }
-
-const char* unsupported_geometry_text() {
-    return "transform lengths must be in {16,32,64,96,128,192,256}; non-cubic grids only with lengths <= 64";
-}
-
-bool geometry_supported(const Geometry& g) {
-    if (!length_supported(g.ta) || !length_supported(g.tb) || !length_supported(g.tc)) return false;
-    if (g.ta == g.tb && g.tb == g.tc) return true;
-    return g.ta <= 64 && g.tb <= 64 && g.tc <= 64;
+    return false;
 }
 
 }  // namespace exx

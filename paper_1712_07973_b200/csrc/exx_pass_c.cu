@@ -1,12 +1,17 @@
-// exx_pass_c.cu -- instantiation + dispatch of pass C (inverse b stage, inverse c-axis FFT, K psi / energy epilogue).
+// exx_pass_c.cu -- instantiation + dispatch of pass C (inverse b stage, inverse c-axis FFT, K psi / energy epilogue) for
+// ONE middle-axis length: compiled once per length with -DEXX_TB=<length> (see exx_inst.cuh).
 #include "exx_inst.cuh"
 #include "exx_launch.h"
 
+#ifndef EXX_TB
+#error "compile with -DEXX_TB=<middle-axis transform length>"
+#endif
+
 namespace exx {
 
-template <int TC, int TB, bool FREE>
-static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
-    using T = TuneAC<TC, TB, FREE>;
+template <int TC, int TB, bool FREE, int CHUNK>
+static cudaError_t run_c_chunk(const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+    using T = TuneAC<TC, TB, FREE, CHUNK>;
     using C = typename T::CfgC;
     constexpr int smem = T::SMEM_C;
     static_assert(smem == T::NBUF_C * C::SMEM_C * 16 + (T::NSTG_C * C::OP_DOUBLES + C::RES_DOUBLES) * 8, "pass C shared memory");
@@ -25,23 +30,28 @@ static cudaError_t run_c(const ArgsAC& args, cudaStream_t s, KernelInfo* info, b
     return cudaGetLastError();
 }
 
-static cudaError_t dispatch_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
-#define X(TC_, TB_)                                                                                  \
-    if (g.tc == TC_ && g.tb == TB_)                                                                  \
-        return g.free_bc ? run_c<TC_, TB_, true>(args, s, info, launch) : run_c<TC_, TB_, false>(args, s, info, launch);
-    EXX_FOR_EACH_PAIR(X)
-#undef X
+template <int TC, int TB, bool FREE>
+static cudaError_t run_c(int chunk, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+    if constexpr (chunk_possible<TB, FREE, 4>()) { if (chunk == 4) return run_c_chunk<TC, TB, FREE, 4>(args, s, info, launch); }
+    if constexpr (chunk_possible<TB, FREE, 2>()) { if (chunk == 2) return run_c_chunk<TC, TB, FREE, 2>(args, s, info, launch); }
+    if constexpr (chunk_possible<TB, FREE, 1>()) { if (chunk == 1) return run_c_chunk<TC, TB, FREE, 1>(args, s, info, launch); }
     return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info) {
-    return dispatch_c(g, args, s, info, true);
-}
-
-cudaError_t query_pass_c(const Geometry& g, KernelInfo* info) {
-    ArgsAC args{};
-    args.na = g.free_bc ? g.ta / 2 : g.ta;
-    return dispatch_c(g, args, nullptr, info, false);
+bool EXX_CAT(try_pass_c_, EXX_TB)(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch, cudaError_t* err) {
+    if (g.tb != EXX_TB) return false;
+#define X(TC_)                                                                                                       \
+    if (g.tc == TC_) {                                                                                               \
+        *err = g.free_bc ? run_c<TC_, EXX_TB, true>(g.chunk, args, s, info, launch) : run_c<TC_, EXX_TB, false>(g.chunk, args, s, info, launch); \
+        return true;                                                                                                 \
+    }
+    if constexpr (is_main_length(EXX_TB)) {
+        EXX_MAIN_LENGTHS(X)
+    } else {
+        X(EXX_TB)
+    }
+#undef X
+    return false;
 }
 
 }  // namespace exx

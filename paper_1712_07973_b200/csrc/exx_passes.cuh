@@ -40,29 +40,25 @@
 namespace exx {
 
 // ---------------------------------------------------------------------------------------- compile-time splits
-template <int T> struct Split;      // line FFT inside a tile: T = P*Q
-template <> struct Split<16>  { static constexpr int P = 4,  Q = 4;  };
-template <> struct Split<32>  { static constexpr int P = 4,  Q = 8;  };
-template <> struct Split<64>  { static constexpr int P = 8,  Q = 8;  };
-template <> struct Split<96>  { static constexpr int P = 8,  Q = 12; };
-template <> struct Split<128> { static constexpr int P = 8,  Q = 16; };
-template <> struct Split<192> { static constexpr int P = 12, Q = 16; };
-template <> struct Split<256> { static constexpr int P = 16, Q = 16; };
-
-template <int T> struct BSplit;     // middle axis split across passes: T = R1*R2 (R1 in pass A/C, R2 in pass B)
-template <> struct BSplit<16>  { static constexpr int R1 = 4,  R2 = 4;  };
-template <> struct BSplit<32>  { static constexpr int R1 = 8,  R2 = 4;  };
-template <> struct BSplit<64>  { static constexpr int R1 = 8,  R2 = 8;  };
-template <> struct BSplit<96>  { static constexpr int R1 = 8,  R2 = 12; };
-template <> struct BSplit<128> { static constexpr int R1 = 16, R2 = 8;  };
-template <> struct BSplit<192> { static constexpr int R1 = 12, R2 = 16; };   // 12 lines per A/C tile: two CTAs per SM
-template <> struct BSplit<256> { static constexpr int R1 = 16, R2 = 16; };
-
-constexpr int r2_of(int tb) {
-    return tb == 16 ? 4 : tb == 32 ? 4 : tb == 64 ? 8 : tb == 96 ? 12 : tb == 128 ? 8 : tb == 192 ? BSplit<192>::R2 : 16;
+// Transform lengths T = 2^a 3^b the FFT covers (reading A9).  "Main" lengths may be mixed freely over the
+// three axes; the "extra" ones are compiled for cubic transform grids only.
+//   line FFT inside a tile:  T = P * Q   (stage 1: P-point in registers, stage 2: Q-point)
+//   middle axis across passes: T = R1 * R2 (R1-point stage in passes A / C, R2-point stage in pass B)
+constexpr bool is_main_length(int t) { return t == 16 || t == 32 || t == 48 || t == 64 || t == 96 || t == 128 || t == 144 || t == 192 || t == 256; }
+constexpr bool is_extra_length(int t) { return t == 24 || t == 72; }
+constexpr bool is_length(int t) { return is_main_length(t) || is_extra_length(t); }
+constexpr int split_p(int t) {
+    return t == 16 ? 4 : t == 24 ? 2 : t == 32 ? 4 : t == 48 ? 4 : t == 64 ? 8 : t == 72 ? 6 : t == 96 ? 8 : t == 128 ? 8 : t == 144 ? 12 :
+           t == 192 ? 12 : t == 256 ? 16 : 0;
 }
-constexpr int split_p(int t) { return t == 16 ? 4 : t == 32 ? 4 : t == 64 ? 8 : t == 96 ? 8 : t == 128 ? 8 : t == 192 ? 12 : 16; }
-constexpr int split_q(int t) { return t / split_p(t); }
+constexpr int split_q(int t) { return split_p(t) ? t / split_p(t) : 0; }
+constexpr int r1_of(int tb) {     // 192 = 12 * 16: 12 lines per A/C tile, two CTAs per SM
+    return tb == 16 ? 4 : tb == 24 ? 2 : tb == 32 ? 8 : tb == 48 ? 4 : tb == 64 ? 8 : tb == 72 ? 6 : tb == 96 ? 8 : tb == 128 ? 16 :
+           tb == 144 ? 12 : tb == 192 ? 12 : tb == 256 ? 16 : 0;
+}
+constexpr int r2_of(int tb) { return r1_of(tb) ? tb / r1_of(tb) : 0; }
+template <int T> struct Split  { static constexpr int P = split_p(T), Q = split_q(T); static_assert(is_length(T), "unsupported transform length"); };
+template <int T> struct BSplit { static constexpr int R1 = r1_of(T), R2 = r2_of(T); static_assert(is_length(T), "unsupported transform length"); };
 constexpr int chunk_for(int ta, int tb, bool free_bc);     // defined after the pass-B geometry helpers
 
 // One packed transform of a same-(j,l) batch: the streamed orbital i forms the pairs (j,i) [real part] and (l,i)
@@ -420,8 +416,8 @@ constexpr int smem_b_bytes(int ta, int tb, bool free_bc, int chunk) {
 }
 constexpr int kMaxSmemB = 224 * 1024;
 // W1 stores CHUNK consecutive (scrambled) c-positions contiguously: the largest of 4, 2, 1 for which the pass-B work +
-// landing buffers of a (TA x R2 x CHUNK)-point block fit shared memory.  Non-cubic grids are limited to lengths <= 64,
-// where the answer is 4 for every combination, so passes A/C may evaluate it with TA := TC.
+// landing buffers of a (TA x R2 x CHUNK)-point block fit shared memory.  It depends on (TA, TB); passes A / C are
+// instantiated for every value it can take for their TB (exx_inst.cuh chunk_possible).
 constexpr int chunk_for(int ta, int tb, bool free_bc) {
     return smem_b_bytes(ta, tb, free_bc, 4) <= kMaxSmemB ? 4 : smem_b_bytes(ta, tb, free_bc, 2) <= kMaxSmemB ? 2 : 1;
 }

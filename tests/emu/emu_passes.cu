@@ -192,5 +192,16 @@ extern "C" int exx_emu_batch(int variant, int ta, int tb, int tc, int free_bc, i
     EMU_CASE(16, 256, 16, 1, 1, 2)
     EMU_CASE(256, 16, 16, 0, 1, 2)
     EMU_CASE(16, 16, 256, 1, 1, 2)
+    EMU_CASE(48, 48, 48, 0, 3, 4)
+    EMU_CASE(48, 16, 16, 1, 1, 4)
+    EMU_CASE(16, 48, 16, 1, 2, 2)
+    EMU_CASE(16, 16, 48, 0, 1, 4)
+    EMU_CASE(144, 16, 16, 0, 1, 4)
+    EMU_CASE(16, 144, 16, 1, 3, 2)
+    EMU_CASE(16, 16, 144, 1, 1, 4)
+    EMU_CASE(24, 24, 24, 0, 2, 4)
+    EMU_CASE(24, 24, 24, 1, 3, 2)
+    EMU_CASE(72, 72, 72, 1, 2, 4)
+    EMU_CASE(72, 72, 72, 0, 1, 2)
     return -1;
 }

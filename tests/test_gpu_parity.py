@@ -184,6 +184,28 @@ def test_every_length(bc, n, n_orb):
     _check_full(w, occ=[2.0, 1.0, 1.5, 0.5][:n_orb], symmetric=True)
 
 
+# ------------------------------------------------------------------ lengths and mixes added in round 2 (reading A9)
+@pytest.mark.parametrize("bc,dims,n_orb", [("periodic", (48, 48, 48), 4), ("periodic", (144, 144, 144), 3), ("free", (24, 24, 24), 4),
+                                           ("free", (72, 72, 72), 3), ("periodic", (24, 24, 24), 5), ("free", (12, 12, 12), 4),
+                                           ("periodic", (72, 72, 72), 3), ("free", (36, 36, 36), 3)])
+def test_new_lengths(bc, dims, n_orb):
+    """Transform lengths 48 = 4*12, 144 = 12*12 (main: free mixes too) and 24 = 2*12, 72 = 6*12 (cubic transform grids)."""
+    base = "C1" if bc == "periodic" else "C2"
+    w = make_workload(small_spec(base, dims=dims, n_orb=n_orb, spacing=(0.3, 0.35, 0.3), number=400 + sum(dims)))
+    _check_full(w, occ=[2.0, 1.0, 1.5, 0.5, 0.7][:n_orb], symmetric=True, batch=2)
+
+
+@pytest.mark.parametrize("bc,dims,n_orb", [("periodic", (96, 128, 192), 3), ("periodic", (192, 96, 48), 3), ("periodic", (16, 256, 144), 3),
+                                           ("free", (64, 96, 128), 2), ("free", (96, 16, 72), 3), ("free", (24, 128, 48), 3),
+                                           ("periodic", (256, 32, 96), 3)])
+def test_noncubic_large_grids(bc, dims, n_orb):
+    """Non-cubic grids with lengths above 64 on every axis role (a: pass B lines, b: split middle axis, c: contiguous):
+    each (TA, TB) picks its own W1 chunk, each (TC, TB, chunk) its own pass A / C instantiation."""
+    base = "C1" if bc == "periodic" else "C2"
+    w = make_workload(small_spec(base, dims=dims, n_orb=n_orb, spacing=(0.3, 0.35, 0.4), number=450 + sum(dims)))
+    _check_full(w, occ=[2.0, 1.0, 1.5][:n_orb], symmetric=True, batch=2)
+
+
 # ------------------------------------------------------------------ large lengths, multi-batch block-rows, element by element
 @pytest.mark.parametrize("bc,n,n_orb,batch", [("periodic", 192, 9, 4), ("free", 128, 9, 4)])
 def test_large_lengths_multibatch_full(bc, n, n_orb, batch):

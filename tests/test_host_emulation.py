@@ -22,11 +22,12 @@ SRC = os.path.join(HERE, "emu", "emu_passes.cu")
 LIB = os.path.join(HERE, "emu", "libexx_emu.so")
 CSRC = os.path.join(ROOT, "paper_1712_07973_b200", "csrc")
 
-SPLIT = {16: (4, 4), 32: (4, 8), 64: (8, 8), 96: (8, 12), 128: (8, 16), 192: (12, 16), 256: (16, 16)}
+SPLIT = {16: (4, 4), 24: (2, 12), 32: (4, 8), 48: (4, 12), 64: (8, 8), 72: (6, 12), 96: (8, 12), 128: (8, 16), 144: (12, 12), 192: (12, 16),
+         256: (16, 16)}
 
 
 def _build():
-    deps = [SRC] + [os.path.join(CSRC, f) for f in ("exx_passes.cuh", "exx_dft.cuh")]
+    deps = [SRC] + [os.path.join(CSRC, f) for f in ("exx_passes.cuh", "exx_dft.cuh", "exx_async.cuh")]
     if os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in deps):
         return LIB
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
@@ -62,6 +63,10 @@ CASES = [
     (16, 32, 64, 0, 2, 4), (64, 16, 32, 1, 4, 4), (16, 96, 16, 1, 3, 2), (16, 16, 128, 0, 1, 4), (128, 16, 16, 1, 1, 4),
     (16, 192, 16, 0, 1, 4), (192, 16, 16, 0, 1, 4), (16, 16, 192, 1, 1, 4), (16, 256, 16, 1, 1, 2),
     (256, 16, 16, 0, 1, 2), (16, 16, 256, 1, 1, 2), (96, 96, 96, 0, 2, 4),
+    # lengths added in round 2 (radix-3 heavy: 48 = 4*12, 144 = 12*12, 24 = 2*12, 72 = 6*12) on every axis role
+    (48, 48, 48, 0, 3, 4), (48, 16, 16, 1, 1, 4), (16, 48, 16, 1, 2, 2), (16, 16, 48, 0, 1, 4),
+    (144, 16, 16, 0, 1, 4), (16, 144, 16, 1, 3, 2), (16, 16, 144, 1, 1, 4), (24, 24, 24, 0, 2, 4), (24, 24, 24, 1, 3, 2),
+    (72, 72, 72, 1, 2, 4), (72, 72, 72, 0, 1, 2),
 ]
 
 

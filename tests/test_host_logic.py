@@ -16,7 +16,7 @@ GOLDEN = os.path.join(ROOT, "tests", "golden")
 def test_library_loads_and_exports_every_declared_symbol():
     lib = exx.load_library()
     header = open(os.path.join(ROOT, "include", "exx.h")).read()
-    declared = set(re.findall(r"\b(exx_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(exx_[a-z0-9_]+)\s*\(", header))
     declared -= {"exx_plan", "exx_status", "exx_bc"}
     assert declared, "no declarations found in include/exx.h"
     for name in sorted(declared):
@@ -89,8 +89,13 @@ def test_status_codes_without_compute():
     sp_bad = (C.c_double * 3)(0.4, -1.0, 0.4)
     assert lib.exx_plan_create(C.byref(h), d, sp_bad, 0, None, 4, None) == 1
     assert lib.exx_plan_create(C.byref(h), d, sp, 0, None, 0, None) == 1          # max_orbitals < 1
-    d = (C.c_int * 3)(32, 64, 96)                                                 # mixed lengths only up to 64
+    d = (C.c_int * 3)(32, 64, 72)                                                 # 24 and 72 only as cubic transform grids
     assert lib.exx_plan_create(C.byref(h), d, sp, 0, None, 4, None) == 2
+    d = (C.c_int * 3)(512, 512, 512)                                              # longer than any compiled length
+    assert lib.exx_plan_create(C.byref(h), d, sp, 0, None, 4, None) == 2
+    d = (C.c_int * 3)(36, 16, 16)                                                 # free BC: 2n = 72 mixed with 32
+    g = np.ones(36 * 16 * 16)
+    assert lib.exx_plan_create(C.byref(h), d, sp, 1, g.ctypes.data_as(C.POINTER(C.c_double)), 4, None) == 2
     assert lib.exx_plan_destroy(None) == 0
     assert lib.exx_plan_workspace_bytes(None) == 0
 
@@ -115,3 +120,44 @@ def test_product_does_not_import_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", src, re.M), f
                 assert "exx_oracle" not in src, f
+
+
+@pytest.mark.parametrize("occ_res,occ_str,max_batch", [([2.0, 1.0, 0.0], [1.0, 0.0, 2.0, 0.5], 0), ([0.0, 0.0], [0.0, 1.0, 0.0], 2),
+                                                       ([1.0], [2.0] * 5, 2), (None, [1.0, 0.0, 2.0], 0)])
+def test_block_schedule_covers_the_rectangle_exactly_once(occ_res, occ_str, max_batch):
+    """Rectangular schedule of exx_apply_block / exx_apply_to (include/exx.h exx_schedule_list_block): every pair
+    (resident j, streamed i) that is not doubly empty appears once; exx_apply_to (no resident occupations) skips the
+    streamed orbitals with f = 0, which contribute nothing to K phi."""
+    n_res = 3 if occ_res is None else len(occ_res)
+    rows = exx.exx_schedule_list_block(occ_res, occ_str, n_res=n_res, max_batch=max_batch)
+    seen = {}
+    per_batch = {}
+    for j, l, i, flags, b in rows.tolist():
+        assert flags in (1, 2, 3) and 0 <= j < n_res and (l == -1 or l == j + 1) and 0 <= i < len(occ_str)
+        per_batch.setdefault(b, []).append((j, l, i))
+        if flags & 1:
+            seen[(j, i)] = seen.get((j, i), 0) + 1
+        if flags & 2:
+            seen[(l, i)] = seen.get((l, i), 0) + 1
+    if occ_res is None:
+        expect = {(j, i) for j in range(n_res) for i in range(len(occ_str)) if occ_str[i] != 0}
+    else:
+        expect = {(j, i) for j in range(n_res) for i in range(len(occ_str)) if not (occ_res[j] == 0 and occ_str[i] == 0)}
+    assert set(seen) == expect and all(v == 1 for v in seen.values())
+    for items in per_batch.values():
+        assert len({(j, l) for j, l, _ in items}) == 1
+        assert len({i for _, _, i in items}) == len(items)
+        if max_batch > 0:
+            assert len(items) <= max_batch
+
+
+def test_masked_schedule_lists_exactly_the_masked_pairs():
+    occ = [2.0, 0.0, 1.0, 0.0, 1.5]
+    n = len(occ)
+    mask = np.zeros((n, n), dtype=np.uint8)
+    for a, b in [(0, 0), (0, 2), (1, 3), (1, 4), (3, 4), (2, 2)]:        # (1,3) is doubly empty: skipped although listed
+        mask[a, b] = mask[b, a] = 1
+    rows = exx.exx_schedule_list(occ, 2, pair_mask=mask)
+    got = sorted([(j, i) for j, l, i, f, b in rows.tolist() if f & 1] + [(l, i) for j, l, i, f, b in rows.tolist() if f & 2])
+    assert got == [(0, 0), (0, 2), (1, 4), (2, 2), (3, 4)]
+    assert np.array_equal(exx.exx_schedule_list(occ, 3, pair_mask=np.ones((n, n))), exx.exx_schedule_list(occ, 3))
