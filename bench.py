@@ -73,8 +73,11 @@ def aggregate_over_ranks(step_ms_local: float, pairs_per_rank: int, world: int, 
     return step_ms, pairs_per_rank * world / (step_ms * 1e-3)
 
 
-def effective_counts(config: str, steps, warmup):
-    """(steps, warmup) actually run for a config given the requested ones (None = default)."""
+def effective_counts(config: str, steps, warmup, quick=False):
+    """(steps, warmup) actually run for a config given the requested ones (None = default).  quick: one warm-up step and
+    one timed step -- for runs under a profiler, whose printed numbers are never bench values."""
+    if quick:
+        return 1, 1
     k = DEFAULT_STEPS[config] if steps is None else max(1, min(int(steps), STEP_CAP[config]))
     w = max(3, min(int(warmup), WARMUP_CAP[config]))                      # timing rule: at least three warm-up steps
     return k, w
@@ -143,7 +146,7 @@ def nominal_flops_per_transform(spec):
     n = spec.dims
     free = spec.bc == "free"
     t = [2 * d for d in n] if free else list(n)
-    r2 = {16: 4, 32: 4, 64: 8, 96: 12, 128: 8, 192: 16, 256: 16}.get(t[1], 16)
+    r2 = {16: 4, 24: 12, 32: 4, 48: 12, 64: 8, 72: 12, 96: 12, 128: 8, 144: 12, 192: 16, 256: 16}.get(t[1], 16)
     r1 = t[1] // r2
     lg = np.log2
     lines_c = n[0] * n[1]                       # non-zero lines along c
@@ -472,7 +475,7 @@ def run_ours(args, rank, local_rank, world):
         torch.cuda.empty_cache()
 
     # ---- the headline configuration
-    steps, warmup = effective_counts(args.config, args.steps, args.warmup)
+    steps, warmup = effective_counts(args.config, args.steps, args.warmup, args.quick)
     res, st = measure_resident(args.config, steps, warmup, local_rank, barrier, args.batch)
     spec = res["spec"]
     step_ms, value = aggregate_over_ranks(res["step_ms_local"], res["n_pairs"], world, all_reduce_max if distributed else None)
@@ -547,6 +550,8 @@ def run_ours(args, rank, local_rank, world):
                 "apply_seconds": step_ms * 1e-3, "E_x": res["E_x"], "clocks": res["clocks"], "gpu_launches": res["launches"],
                 "e2e": e2e, "roofline": roofline, "roofline_path": roofline_path, "fp64_peak_measured": fp64,
                 "per_config": per_config, "cpu_baseline": cpu, "cufft_comparison": cufft}
+        if args.quick:
+            line["quick"] = "profiling run (1 warm-up step, 1 timed step): not a bench value"
         print(json.dumps(line))
     plan.destroy()
     if distributed:
@@ -614,9 +619,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the C3 / C4 lines of per_config")
+    ap.add_argument("--quick", action="store_true", help="profiling runs: 1 warm-up + 1 timed step, no per_config / e2e / cpu_baseline")
     ap.add_argument("--compare-cufft", action="store_true", help="also time a torch.fft (cuFFT) pipeline on a sample, as a comparison")
     args = ap.parse_args()
 
+    if args.quick:
+        args.no_per_config = args.no_e2e = args.no_cpu_baseline = True
     rank, local_rank, world, spawn = rank_env(args.gpus)
     if spawn and args.impl == "ours":
         # plain `python bench.py --gpus N`: start the N ranks here (what torchrun would do), one process per GPU
