@@ -328,7 +328,7 @@ def run_reference(args, rank, world):
 
 
 # ------------------------------------------------------------------------------------------------ the product arm
-def measure_resident(name, steps, warmup, local_rank, barrier, batch=0):
+def measure_resident(name, steps, warmup, local_rank, barrier, batch=0, n_orb=0):
     """Device-resident measurement of one configuration.  Returns (result dict, state) where state keeps the workload,
     the plan and the device tensors alive for the caller (e2e, cpu_baseline, cuFFT comparison)."""
     import torch
@@ -336,6 +336,9 @@ def measure_resident(name, steps, warmup, local_rank, barrier, batch=0):
     import paper_1712_07973_b200 as exx
     from workloads import CONFIGS, make_workload
     spec = CONFIGS[name]
+    if n_orb > 0:                                                   # development runs only: same grid, fewer orbitals
+        from workloads import small_spec
+        spec = small_spec(name, n_orb=n_orb, name=f"{name}-dev{n_orb}", orthonormalize=False)
     w = make_workload(spec, device="cuda")
     psi, occ = w["psi"], w["occ"]
     kpsi = torch.empty_like(psi)
@@ -476,7 +479,7 @@ def run_ours(args, rank, local_rank, world):
 
     # ---- the headline configuration
     steps, warmup = effective_counts(args.config, args.steps, args.warmup, args.quick)
-    res, st = measure_resident(args.config, steps, warmup, local_rank, barrier, args.batch)
+    res, st = measure_resident(args.config, steps, warmup, local_rank, barrier, args.batch, args.dev_orbitals)
     spec = res["spec"]
     step_ms, value = aggregate_over_ranks(res["step_ms_local"], res["n_pairs"], world, all_reduce_max if distributed else None)
     roofline, roofline_path = roofline_objects(res, step_ms, fp64)
@@ -550,6 +553,8 @@ def run_ours(args, rank, local_rank, world):
                 "apply_seconds": step_ms * 1e-3, "E_x": res["E_x"], "clocks": res["clocks"], "gpu_launches": res["launches"],
                 "e2e": e2e, "roofline": roofline, "roofline_path": roofline_path, "fp64_peak_measured": fp64,
                 "per_config": per_config, "cpu_baseline": cpu, "cufft_comparison": cufft}
+        if args.dev_orbitals:
+            line["dev"] = f"development run with {args.dev_orbitals} orbitals instead of the configuration's: not a bench value"
         if args.quick:
             line["quick"] = "profiling run (1 warm-up step, 1 timed step): not a bench value"
         print(json.dumps(line))
@@ -620,10 +625,11 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the C3 / C4 lines of per_config")
     ap.add_argument("--quick", action="store_true", help="profiling runs: 1 warm-up + 1 timed step, no per_config / e2e / cpu_baseline")
+    ap.add_argument("--dev-orbitals", type=int, default=0, help="development runs: the configuration's grid with this many orbitals (not a bench value)")
     ap.add_argument("--compare-cufft", action="store_true", help="also time a torch.fft (cuFFT) pipeline on a sample, as a comparison")
     args = ap.parse_args()
 
-    if args.quick:
+    if args.quick or args.dev_orbitals:
         args.no_per_config = args.no_e2e = args.no_cpu_baseline = True
     rank, local_rank, world, spawn = rank_env(args.gpus)
     if spawn and args.impl == "ours":

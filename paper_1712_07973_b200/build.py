@@ -50,9 +50,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = _nvcc()
     os.makedirs(OBJ, exist_ok=True)
 
+    hdr_time = max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS + [os.path.basename(__file__)] if os.path.exists(os.path.join(CSRC, h)))
+    hdr_time = max(hdr_time, os.path.getmtime(os.path.abspath(__file__)))
+
     def compile_one(unit) -> str:
         src, defines, objname = unit
         obj = os.path.join(OBJ, objname)
+        # incremental: an object newer than its source, every header and this script is kept (same build mode only)
+        if not force and same_mode and os.path.exists(obj) and os.path.getmtime(obj) >= max(hdr_time, os.path.getmtime(os.path.join(CSRC, src))):
+            return obj
         cmd = [nvcc] + ARCH + FLAGS + DEV_FLAGS + defines + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose:
@@ -64,7 +70,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     with ThreadPoolExecutor(max_workers=max(1, min(len(UNITS), os.cpu_count() or 4))) as ex:
         objs = list(ex.map(compile_one, UNITS))
-    r = subprocess.run([nvcc] + ARCH + ["-shared", "-o", LIB] + objs, capture_output=True, text=True)
+    r = subprocess.run([nvcc] + ARCH + ["-shared", "-o", LIB] + objs + ["-ldl"], capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     with open(mode_file, "w") as fh:

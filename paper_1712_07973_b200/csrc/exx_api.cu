@@ -12,6 +12,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; the ranges cost nothing unless a tool (nsys, ncu --nvtx) attaches
+
 #include "../../include/exx.h"
 #include "exx_launch.h"
 #include "exx_sched.hpp"
@@ -514,7 +516,14 @@ exx_status run_job_unguarded(exx_plan* p, const Job& job) {
 
 // No exception crosses the C ABI: the schedule vectors are reserved at plan creation, so nothing in the hot path
 // allocates, and anything that throws all the same is turned into a status code here.
+struct NvtxRange {                                          // one named range per apply on the tools' timeline
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+
 exx_status run_job(exx_plan* p, const Job& job) {
+    NvtxRange range(job.square ? (job.mask ? "exx_apply_pairs" : (job.kpsi_host ? "exx_apply_host" : "exx_apply"))
+                               : (job.kpsi_str ? "exx_apply_block" : "exx_apply_to"));
     exx_status st;
     try {
         st = run_job_unguarded(p, job);

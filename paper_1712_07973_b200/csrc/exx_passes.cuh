@@ -536,15 +536,19 @@ EXX_HD void b1_compute(double2* colp, const double2* tw, int tws) {
 // ---- B2: last forward stage along a, multiply by K^ ("convolving the density with the appropriate
 //      Green's function"), first inverse stage along a.  kcol = K^ line [sa] of this column (symmetric a index);
 //      conj twiddle W_TA^{-n2 k1} = conj(tw[n2*tws]).
+// K^ values of one B2 item (frequencies ka = k1 + PA k2, symmetric index): issued well before they are used so that
+// the L2 latency hides behind the FFT stages in between
 template <class C>
-EXX_HD void b2_compute(double2* colp, const double* kcol, const double2* tw, int tws, int k1) {
-    double xr[C::QA], xi[C::QA];
-    double kv[C::QA];                                          // issued first: the L2 latency hides behind the forward DFT
+EXX_HD void b2_load_k(const double* kcol, int k1, double* kv /*[QA]*/) {
 #pragma unroll
     for (int k2 = 0; k2 < C::QA; ++k2) {
         const int ka = k1 + C::PA * k2;
         kv[k2] = ld_ro(kcol + (ka <= C::TA - ka ? ka : C::TA - ka));
     }
+}
+template <class C>
+EXX_HD void b2_compute(double2* colp, const double* kv, const double2* tw, int tws, int k1) {
+    double xr[C::QA], xi[C::QA];
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = colp[n2 * C::RS]; xr[n2] = v.x; xi[n2] = v.y; }
     Dft<C::QA>::run(xr, xi);
@@ -597,14 +601,8 @@ EXX_HD void b1e_compute(const double2* in, double2* out, const double2* tw, int 
     }
 }
 template <class C>
-EXX_HD void b2e_compute(double2* colp, const double* kcol, const double2* tw, int tws, int k1) {
+EXX_HD void b2e_compute(double2* colp, const double* kv, const double2* tw, int tws, int k1) {
     double xr[C::QA], xi[C::QA];
-    double kv[C::QA];
-#pragma unroll
-    for (int k2 = 0; k2 < C::QA; ++k2) {
-        const int ka = k1 + C::PA * k2;
-        kv[k2] = ld_ro(kcol + (ka <= C::TA - ka ? ka : C::TA - ka));
-    }
 #pragma unroll
     for (int n2 = 0; n2 < C::QA; ++n2) { double2 v = colp[n2 * C::NCW]; xr[n2] = v.x; xi[n2] = v.y; }
     Dft<C::QA>::run(xr, xi);
@@ -877,7 +875,9 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
                     const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
                     const int kb = q + C::R1 * r;
                     const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-                    b2_compute<C>(W + x.base, g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA, TW2 + x.k, C::PA, x.k);
+                    double kv[C::QA];
+                    b2_load_k<C>(g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA, x.k, kv);
+                    b2_compute<C>(W + x.base, kv, TW2 + x.k, C::PA, x.k);
                 }
             __syncwarp();
 #pragma unroll
@@ -1007,6 +1007,17 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
             mbar_wait(&ready[k & 1], (k >> 1) & 1);
             for (int cg = wid; cg < C::NGRP; cg += NY) {
                 double2* const E = ESC + wid * C::E_ELEMS;
+                // K^ of this lane's B2 item: with one item per lane (NP = 1) the loads are issued here, ahead of B1, so
+                // that their L2 latency hides behind B1 and the forward half of B2
+                double kv0[C::QA];
+                auto kcol_of = [&](int w) {
+                    const ColAIdx x = colp_index<C>(cg, w);
+                    const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
+                    const int kb = q + C::R1 * r;
+                    const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
+                    return g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA;
+                };
+                if (NP == 1 && lane < C::ITEMS_P) b2_load_k<C>(kcol_of(lane), colp_index<C>(cg, lane).k, kv0);
 #pragma unroll
                 for (int m = 0; m < NQ; ++m)
                     if (lane + m * 32 < C::ITEMS_Q) {
@@ -1021,12 +1032,11 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
                     if (lane + m * 32 < C::ITEMS_P) {
                         const int w = lane + m * 32;
                         const ColAIdx x = colp_index<C>(cg, w);
-                        const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
-                        const int kb = q + C::R1 * r;
-                        const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-                        const double* kcol = g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA;
-                        if (SCRATCH) b2e_compute<C>(E + x.k * C::QRSE + w % C::NCW, kcol, TW2 + x.k, C::PA, x.k);
-                        else b2_compute<C>(W + x.base, kcol, TW2 + x.k, C::PA, x.k);
+                        double kvm[C::QA];
+                        if (NP != 1) b2_load_k<C>(kcol_of(w), x.k, kvm);
+                        const double* kv = NP == 1 ? kv0 : kvm;
+                        if (SCRATCH) b2e_compute<C>(E + x.k * C::QRSE + w % C::NCW, kv, TW2 + x.k, C::PA, x.k);
+                        else b2_compute<C>(W + x.base, kv, TW2 + x.k, C::PA, x.k);
                     }
                 __syncwarp();
 #pragma unroll

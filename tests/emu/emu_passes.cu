@@ -86,7 +86,9 @@ static int emu_batch(bool scratch, const double* psi, double* kpsi, int j, int l
                     const int r = x.col / CHUNK, pin = x.col % CHUNK;
                     const int kb = q + B::R1 * r;
                     const int sb = kb <= TB - kb ? kb : TB - kb;
-                    b2_compute<B>(W.data() + x.base, ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, twa2.data() + x.k, B::PA, x.k);
+                    double kv[B::QA];
+                    b2_load_k<B>(ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, x.k, kv);
+                    b2_compute<B>(W.data() + x.base, kv, twa2.data() + x.k, B::PA, x.k);
                 }
                 for (int w = 0; w < B::ITEMS_Q; ++w) b3_compute<B>(W.data() + colq_index<B>(cg, w).base);
             }
@@ -103,7 +105,9 @@ static int emu_batch(bool scratch, const double* psi, double* kpsi, int j, int l
                     const int r = x.col / CHUNK, pin = x.col % CHUNK;
                     const int kb = q + B::R1 * r;
                     const int sb = kb <= TB - kb ? kb : TB - kb;
-                    b2e_compute<B>(E.data() + x.k * B::QRSE + w % B::NCW, ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, twa2.data() + x.k, B::PA, x.k);
+                    double kv[B::QA];
+                    b2_load_k<B>(ks.data() + (static_cast<size_t>(sb) * TC + pch * CHUNK + pin) * B::NSA, x.k, kv);
+                    b2e_compute<B>(E.data() + x.k * B::QRSE + w % B::NCW, kv, twa2.data() + x.k, B::PA, x.k);
                 }
                 for (int w = 0; w < B::ITEMS_Q; ++w) b3e_compute<B>(E.data() + w, W.data() + colq_index<B>(cg, w).base);
             }
