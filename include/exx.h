@@ -54,8 +54,9 @@ typedef enum { EXX_BC_PERIODIC = 0, EXX_BC_FREE = 1 } exx_bc;
 /*
  * exx_plan_create -- one-time setup for a grid, boundary condition and Green's function (PAPER.md:125:
  * "The Green's function can be discretized for ... free ... and periodic" boundary conditions).
- *   dims        HOST, n1,n2,n3.  Transform length per axis T = n (periodic) or 2n (free); T must be one of
- *               {16, 32, 64, 96, 128, 192, 256} (radix-2/3 only), else EXX_ERR_UNSUPPORTED_SIZE.
+ *   dims        HOST, n1,n2,n3.  Transform length per axis T = n (periodic) or 2n (free); every T must be one of
+ *               {16, 32, 48, 64, 96, 128, 144, 192, 256} (any mix over the three axes), or the transform grid is cubic
+ *               with T = 24 or 72 (radix-2/3 only, reading A9); else EXX_ERR_UNSUPPORTED_SIZE.
  *   spacing     HOST, h1,h2,h3 in bohr (> 0).
  *   bc          EXX_BC_PERIODIC or EXX_BC_FREE.
  *   kernel_host HOST.  PERIODIC: NULL => analytic 4 pi/|G|^2, G = 0 -> 0.  Non-NULL => Fourier-space filter table

@@ -152,6 +152,13 @@ struct TuneAC {
     static constexpr int NSTG_C = two_fit(2, 2) ? 2 : two_fit(1, 2) ? 2 : two_fit(1, 1) ? 1 : one_fits(NBUF_C, 2) ? 2 : 1;
     static constexpr int SMEM_C = smem_ac_bytes<TC, TB, FREE>(G_C, NSTG_C, true, NBUF_C);
     static constexpr int MINB_C = pick_minb(SMEM_C + (TC + TB) * 16 + 256, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
+    // single-buffered pass C: gather the next W1 tile from inside C2 (pass_c_kernel EARLY) where the register file leaves
+    // room for the PC complex inputs of every C2 item next to the accumulators without spilling them
+#ifdef EXX_EARLY_C_ALL
+    static constexpr bool EARLY_C = NBUF_C == 1;
+#else
+    static constexpr bool EARLY_C = NBUF_C == 1 && 65536 / (NT_C * MINB_C) >= 160;
+#endif
     // ---- pass A
     static constexpr int G_A = pick_g<TC, TB, FREE>(false, kMaxSmemAC / 3);
     using CfgA = CfgAC<TC, TB, FREE, G_A, CHUNK>;

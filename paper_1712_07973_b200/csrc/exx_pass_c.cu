@@ -18,7 +18,7 @@ static cudaError_t run_c_chunk(const ArgsAC& args, cudaStream_t s, KernelInfo* i
     static_assert(!T::WS_C || (T::NBUF_C == 2 && T::NSTG_C == 2), "warp-specialised pass C needs two buffers and two stages");
     constexpr bool ws = T::WS_C;
     constexpr int nt = ws ? 32 * (T::NAW_C + T::NBW_C) : T::NT_C;
-    auto kern = ws ? pass_c_ws_kernel<C, T::NAW_C, T::NBW_C, 2, T::MINB_C_WS> : pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C>;
+    auto kern = ws ? pass_c_ws_kernel<C, T::NAW_C, T::NBW_C, 2, T::MINB_C_WS> : pass_c_kernel<C, T::NT_C, T::NSTG_C, T::NBUF_C, T::MINB_C, T::EARLY_C>;
     static LaunchCache cache;
     int occ = 0;
     if (info) { info->threads = nt; info->smem_bytes = smem; info->tiles = args.na * C::TILES_PER_A; info->ctas_per_sm = 0; info->name = ws ? "pass_c_ws_kernel" : "pass_c_kernel"; }

@@ -303,12 +303,17 @@ EXX_HD void c1_compute(double2* seg, const double2* tw, int tws, int k1) {
 //      of K psi_i: the cross term f_j V_jl psi_j of K psi_l goes into accl instead, so every K psi address receives
 //      exactly one reduce-add per launch.
 //      rj / rl = resident psi_j / psi_l lines, oi = operand line, all at the item's first point (stride QC doubles).
+//      The phase comes in two halves so that a single-buffered kernel can release the work buffer early: c2_load reads the
+//      item's PC inputs into registers (after it, nothing of transform t is left in the buffer that this item needs),
+//      c2_finish does the arithmetic.
 template <class C>
-EXX_HD void c2_compute(const double2* row, const XformDesc& d, int l, double fj, double fl, const double* rj, const double* rl,
-                       double* oi, double* accj /*[PCN]*/, double* accl /*[PCN]*/, double& e1, double& e2) {
-    double xr[C::PC], xi[C::PC];
+EXX_HD void c2_load(const double2* row, double* xr /*[PC]*/, double* xi /*[PC]*/) {
 #pragma unroll
     for (int k1 = 0; k1 < C::PC; ++k1) { double2 v = row[k1 * C::QCP]; xr[k1] = v.x; xi[k1] = v.y; }
+}
+template <class C>
+EXX_HD void c2_finish(double* xr, double* xi, const XformDesc& d, int l, double fj, double fl, const double* rj, const double* rl,
+                      double* oi, double* accj /*[PCN]*/, double* accl /*[PCN]*/, double& e1, double& e2) {
     dft_inv<C::PC, C::FREE>(xr, xi);
     const double m1 = (d.flags & 1) ? 1.0 : 0.0, m2 = (d.flags & 2) ? 1.0 : 0.0;
     const double fjl = d.i == l ? fj : 0.0;
@@ -328,6 +333,13 @@ EXX_HD void c2_compute(const double2* row, const XformDesc& d, int l, double fj,
     }
     e1 += s1;
     e2 += s2;
+}
+template <class C>
+EXX_HD void c2_compute(const double2* row, const XformDesc& d, int l, double fj, double fl, const double* rj, const double* rl,
+                       double* oi, double* accj /*[PCN]*/, double* accl /*[PCN]*/, double& e1, double& e2) {
+    double xr[C::PC], xi[C::PC];
+    c2_load<C>(row, xr, xi);
+    c2_finish<C>(xr, xi, d, l, fj, fl, rj, rl, oi, accj, accl, e1, e2);
 }
 
 // ---------------------------------------------------------------------------------------- pass B geometry
@@ -1064,8 +1076,11 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
 //   * the K psi_i increment overwrites those lines and leaves by TMA bulk reduce-add (fp64) -- each K psi address
 //     receives exactly one add per launch (the i of a batch are distinct and never j or l), so the result is
 //     deterministic.
-template <class C, int NT, int NSTG, int NBUF, int MINB>
+//   * EARLY (single work buffer only): C2 first takes its inputs into registers, which frees the buffer, and the gather
+//     of transform t+1 is issued from there, so that its latency hides behind the P-point stage and the epilogue of t.
+template <class C, int NT, int NSTG, int NBUF, int MINB, bool EARLY>
 __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
+    static_assert(!EARLY || NBUF == 1, "the early gather is the single-buffer scheme");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* const S0 = reinterpret_cast<double2*>(smem_raw);
     double* const OP = reinterpret_cast<double*>(S0 + NBUF * C::SMEM_C);
@@ -1101,7 +1116,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
                 for (int q = 0; q < C::R1; ++q) cp_async16(dstbuf + c0[m].col + q * C::ROW, w1t + c0[m].w1 + q * qstride);
             }
     };
-    if (NBUF == 2) {
+    if (NBUF == 2 || EARLY) {
         issue_w1_gather(0);
         cp_async_commit();
     }
@@ -1138,6 +1153,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             if (t + 1 < g.count) issue_w1_gather(t + 1);
             cp_async_commit();
             cp_async_wait<1>();                            // this thread's columns of transform t have landed
+        } else if (EARLY) {                                // single work buffer, gather of t issued from inside C2 of t-1
+            cp_async_wait<0>();
         } else {                                           // single work buffer: no overlap of the gather
             issue_w1_gather(t);
             cp_async_commit();
@@ -1151,14 +1168,34 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         for (int m = 0; m < NI1; ++m)
             if (tid + m * NT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, s_twct + p1[m].k1, C::PC, p1[m].k1);
         __syncthreads();
-        if (t == 0) mbar_wait(&resbar, 0);                 // psi_j / psi_l lines of the tile
-        mbar_wait(&full[s], (t / NSTG) & 1);               // psi_i lines of transform t have landed
         double e1 = 0.0, e2 = 0.0;
+        if (!EARLY) {
+            if (t == 0) mbar_wait(&resbar, 0);             // psi_j / psi_l lines of the tile
+            mbar_wait(&full[s], (t / NSTG) & 1);           // psi_i lines of transform t have landed
 #pragma unroll
-        for (int m = 0; m < NI2; ++m)
-            if (tid + m * NT < C::ITEMS_LINE_Q)
-                c2_compute<C>(S + q2[m].row, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
-                              accj[m], accl[m], e1, e2);
+            for (int m = 0; m < NI2; ++m)
+                if (tid + m * NT < C::ITEMS_LINE_Q)
+                    c2_compute<C>(S + q2[m].row, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                                  accj[m], accl[m], e1, e2);
+        } else {
+            // single work buffer: every item first takes its inputs into registers; after the barrier nothing of transform
+            // t is left in the buffer, so the W1 tile of t+1 is gathered into it while the P-point stage and the Kernel-3
+            // epilogue of t run out of registers (the gather latency hides behind them)
+            double xr[NI2][C::PC], xi[NI2][C::PC];
+#pragma unroll
+            for (int m = 0; m < NI2; ++m)
+                if (tid + m * NT < C::ITEMS_LINE_Q) c2_load<C>(S + q2[m].row, xr[m], xi[m]);
+            __syncthreads();
+            if (t + 1 < g.count) issue_w1_gather(t + 1);
+            cp_async_commit();
+            if (t == 0) mbar_wait(&resbar, 0);
+            mbar_wait(&full[s], (t / NSTG) & 1);
+#pragma unroll
+            for (int m = 0; m < NI2; ++m)
+                if (tid + m * NT < C::ITEMS_LINE_Q)
+                    c2_finish<C>(xr[m], xi[m], d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                                 accj[m], accl[m], e1, e2);
+        }
         fence_proxy_async();                               // increments visible to the TMA reads below
         // block reduction of the energy partials in a fixed order (deterministic)
 #pragma unroll
