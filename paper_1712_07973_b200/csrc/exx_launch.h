@@ -154,8 +154,10 @@ struct TuneAC {
     static constexpr int MINB_C = pick_minb(SMEM_C + (TC + TB) * 16 + 256, NT_C, 128, 4, CfgC::NC * CfgC::TILES_PER_A);
     // single-buffered pass C: gather the next W1 tile from inside C2 (pass_c_kernel EARLY) where the register file leaves
     // room for the PC complex inputs of every C2 item next to the accumulators without spilling them
-#ifdef EXX_EARLY_C_ALL
+#if defined(EXX_EARLY_C_ALL)
     static constexpr bool EARLY_C = NBUF_C == 1;
+#elif defined(EXX_EARLY_C_NONE)
+    static constexpr bool EARLY_C = false;
 #else
     static constexpr bool EARLY_C = NBUF_C == 1 && 65536 / (NT_C * MINB_C) >= 160;
 #endif

@@ -659,6 +659,23 @@ __device__ __forceinline__ void issue_operand_loads(const ArgsAC& g, const Xform
     issue_line_loads<C>(g, g.psi, d.i, stage, bar, a, b2base, lane);
 }
 
+// Pass A with a single operand stage (the geometries where a second one would cost the second CTA of an SM): the load
+// of transform t+1 can only be issued once A0 of t has consumed the stage, so its full DRAM latency would sit on the
+// critical path of every iteration.  The lines of transform t+2 are therefore prefetched into L2 at that point (no
+// shared-memory destination): the later bulk copy then meets an L2 hit.  Measured at 192^3: pass A -3 %; the same in
+// pass C (+6 %) and with two stages (256^3 free: pass A +29 %) is slower -- the prefetches compete with the bulk
+// copies and reduce-adds for the TMA unit -- so it stays confined to this case.
+#ifndef EXX_PF_MODE
+#define EXX_PF_MODE 1            // 0: never, 1: pass A with one operand stage, 2: pass A always
+#endif
+template <int NSTG>
+__host__ __device__ constexpr bool prefetch_operands() { return EXX_PF_MODE == 2 || (EXX_PF_MODE == 1 && NSTG == 1); }
+template <class C>
+__device__ __forceinline__ void issue_operand_prefetch(const ArgsAC& g, const XformDesc& d, int a, int b2base, int lane) {
+    const double* base = g.psi + static_cast<size_t>(d.i) * g.m_points;
+    for (int l = lane; l < C::LINES; l += 32) bulk_prefetch_l2(base + line_offset<C>(l, a, b2base), C::LINE_BYTES);
+}
+
 // Pass A.  One CTA per (a, b2-group) tile, looping over the transforms of the same-(j,l) batch.  psi_j and psi_l of the
 // thread's points live in registers; the streamed psi_i lines arrive NSTG transforms ahead by TMA bulk copies.
 template <class C, int NT, int NSTG, int MINB>
@@ -682,6 +699,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
     if (tid < 32)
         for (int t = 0; t < NSTG && t < g.count; ++t)
             issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+    if (prefetch_operands<NSTG>() && tid < 32 && NSTG < g.count) issue_operand_prefetch<C>(g, g.desc[NSTG], a, b2base, tid);
 
     // per-thread items, resolved once
     LineQIdx q0[NI0];
@@ -715,8 +733,10 @@ __global__ void __launch_bounds__(NT, MINB) pass_a_kernel(const ArgsAC g) {
             if (tid + m * NT < C::ITEMS_LINE_Q)
                 a0_compute<C>(vj[m], vl[m], stage + q0[m].op, flags, S + q0[m].row, s_twc + q0[m].n2);
         __syncthreads();
-        if (tid < 32 && t + NSTG < g.count)                    // the stage has been consumed: refill it
+        if (tid < 32 && t + NSTG < g.count) {                  // the stage has been consumed: refill it
             issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+            if (prefetch_operands<NSTG>() && t + NSTG + 1 < g.count) issue_operand_prefetch<C>(g, g.desc[t + NSTG + 1], a, b2base, tid);
+        }
 #pragma unroll
         for (int m = 0; m < NI1; ++m)
             if (tid + m * NT < C::ITEMS_LINE_P) a1_compute<C>(S + p1[m].seg);
@@ -761,6 +781,7 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_a_ws_kernel(const
         if (tid < 32)
             for (int t = 0; t < NSTG && t < g.count; ++t)
                 issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+        if (prefetch_operands<NSTG>() && tid < 32 && NSTG < g.count) issue_operand_prefetch<C>(g, g.desc[NSTG], a, b2base, tid);
         LineQIdx q0[NI0];
         double vj[NI0][C::PCN], vl[NI0][C::PCN];
 #pragma unroll
@@ -790,8 +811,10 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_a_ws_kernel(const
                 if (tid + m * AT < C::ITEMS_LINE_Q)
                     a0_compute<C>(vj[m], vl[m], stage + q0[m].op, flags, S + q0[m].row, s_twc + q0[m].n2);
             asm volatile("bar.sync 1, %0;" ::"n"(AT) : "memory");
-            if (tid < 32 && t + NSTG < g.count)                        // the stage has been consumed: refill it
+            if (tid < 32 && t + NSTG < g.count) {                      // the stage has been consumed: refill it
                 issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+                if (prefetch_operands<NSTG>() && t + NSTG + 1 < g.count) issue_operand_prefetch<C>(g, g.desc[t + NSTG + 1], a, b2base, tid);
+            }
 #pragma unroll
             for (int m = 0; m < NI1; ++m)
                 if (tid + m * AT < C::ITEMS_LINE_P) a1_compute<C>(S + p1[m].seg);
@@ -946,8 +969,16 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
         const int q = rest % C::R1, pch = rest / C::R1;
         return g.w1 + ((static_cast<size_t>(t) * C::R1 + q) * g.npch + pch) * C::BLOCK_ELEMS;
     };
-    const int stride = gridDim.x, id0 = blockIdx.x;
-    const int nk = id0 < g.ntiles ? (g.ntiles - id0 + stride - 1) / stride : 0;
+    // KREUSE (one column group per column warp, one B2 item per lane): every CTA takes a CONTIGUOUS range of block ids
+    // (t fastest), so consecutive blocks of a CTA are the same (q, pch) slice of consecutive transforms and the K^ values
+    // a column-warp lane needs stay in its registers for a whole run of blocks (96^3: pass B -7.5 %).  With two column
+    // groups per warp the values alternate anyway; there the blocks stay interleaved over the CTAs (CTAs that run at the
+    // same time share a K^ slice in L2) and the loads are issued ahead of B1 (measured: contiguous ranges +2..4 %).
+    constexpr bool KREUSE = C::NGRP == NY && NP == 1;
+    const int per_cta = (g.ntiles + static_cast<int>(gridDim.x) - 1) / static_cast<int>(gridDim.x);
+    const int stride = KREUSE ? 1 : static_cast<int>(gridDim.x);
+    const int id0 = KREUSE ? static_cast<int>(blockIdx.x) * per_cta : static_cast<int>(blockIdx.x);
+    const int nk = id0 >= g.ntiles ? 0 : KREUSE ? (g.ntiles - id0 < per_cta ? g.ntiles - id0 : per_cta) : (g.ntiles - id0 + stride - 1) / stride;
 
     if (wid >= NY) {
         // ------------------------------------------------------------------ row warps: landing, B0, B4, refill
@@ -1011,25 +1042,34 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
         if (nk > 0) b4_block(nk - 1);
     } else {
         // ------------------------------------------------------------------ column warps: a-axis phases
+        // K^ of this lane's B2 item (one item per lane, NP = 1) is requested ahead of B1 so that the L2 latency hides
+        // behind it.  KREUSE: nothing is requested when the values in the registers are the right ones already (same
+        // (q, pch) slice: the usual case inside a contiguous run of blocks), and the first block of a new slice requests
+        // its values as soon as B2 of the previous block has consumed the old ones.
+        double kv0[C::QA];
+        int k_slice = -1, k_cg = -1;                       // (q, pch) slice and column group the values in kv0 belong to
+        auto kcol_of = [&](int slice, int cg, int w) {
+            const int q = slice % C::R1, pch = slice / C::R1;
+            const ColAIdx x = colp_index<C>(cg, w);
+            const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
+            const int kb = q + C::R1 * r;
+            const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
+            return g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA;
+        };
+        auto request_k = [&](int slice, int cg) {
+            if (NP != 1 || (slice == k_slice && cg == k_cg)) return;
+            if (lane < C::ITEMS_P) b2_load_k<C>(kcol_of(slice, cg, lane), colp_index<C>(cg, lane).k, kv0);
+            k_slice = slice; k_cg = cg;
+        };
+        if (nk > 0 && wid < C::NGRP) request_k(id0 / g.count, wid);
         for (int k = 0; k < nk; ++k) {
             const int id = id0 + k * stride;
             double2* const W = BUF + (k & 1) * BUF_ELEMS;
-            const int rest = id / g.count;
-            const int q = rest % C::R1, pch = rest / C::R1;
+            const int slice = id / g.count;
             mbar_wait(&ready[k & 1], (k >> 1) & 1);
             for (int cg = wid; cg < C::NGRP; cg += NY) {
                 double2* const E = ESC + wid * C::E_ELEMS;
-                // K^ of this lane's B2 item: with one item per lane (NP = 1) the loads are issued here, ahead of B1, so
-                // that their L2 latency hides behind B1 and the forward half of B2
-                double kv0[C::QA];
-                auto kcol_of = [&](int w) {
-                    const ColAIdx x = colp_index<C>(cg, w);
-                    const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
-                    const int kb = q + C::R1 * r;
-                    const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-                    return g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA;
-                };
-                if (NP == 1 && lane < C::ITEMS_P) b2_load_k<C>(kcol_of(lane), colp_index<C>(cg, lane).k, kv0);
+                request_k(slice, cg);
 #pragma unroll
                 for (int m = 0; m < NQ; ++m)
                     if (lane + m * 32 < C::ITEMS_Q) {
@@ -1045,11 +1085,12 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
                         const int w = lane + m * 32;
                         const ColAIdx x = colp_index<C>(cg, w);
                         double kvm[C::QA];
-                        if (NP != 1) b2_load_k<C>(kcol_of(w), x.k, kvm);
+                        if (NP != 1) b2_load_k<C>(kcol_of(slice, cg, w), x.k, kvm);
                         const double* kv = NP == 1 ? kv0 : kvm;
                         if (SCRATCH) b2e_compute<C>(E + x.k * C::QRSE + w % C::NCW, kv, TW2 + x.k, C::PA, x.k);
                         else b2_compute<C>(W + x.base, kv, TW2 + x.k, C::PA, x.k);
                     }
+                if (KREUSE && k + 1 < nk) request_k((id + stride) / g.count, wid);
                 __syncwarp();
 #pragma unroll
                 for (int m = 0; m < NQ; ++m)
