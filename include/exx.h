@@ -66,6 +66,11 @@ typedef enum { EXX_BC_PERIODIC = 0, EXX_BC_FREE = 1 } exx_bc;
  *               kernel 2 would be different".
  *               FREE: table g[a][b][c] of n1*n2*n3 doubles = Green's function at displacement
  *               (a h1, b h2, c h3), units 1/bohr (an interpolating-scaling-function table can be passed as is).
+ *               SLAB / WIRE boundary conditions ("free, wire, slab and periodic") are FREE plans whose
+ *               table holds ONE FULL PERIOD of the mixed Green's function along each periodic axis (index d <->
+ *               displacement d*h, even under d -> n-d) and displacements 0..n-1 along each isolated axis: zero-padded
+ *               convolution with g[|d|] equals wrap-around convolution on every axis on which g is even-periodic
+ *               (reading A24).
  *               Either table is copied during the call; the caller may free it afterwards.
  *   max_orbitals  upper bound for n_orb of later exx_apply calls (sizes the pair-energy buffers).
  *   cuda_stream cudaStream_t as void* (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream.

@@ -40,6 +40,7 @@ def _load():
         lib.exx_oracle_apply_to.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int, _dp, _dp]
         lib.exx_oracle_apply_block.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp]
         lib.exx_oracle_set_periodic_filter.argtypes = [C.c_void_p, _dp]
+        lib.exx_oracle_poisson_direct_mixed.argtypes = [_ip, _dp, _ip, _dp, _dp, _dp]
         lib.exx_oracle_threads.argtypes = []
         _lib = lib
     return _lib
@@ -244,6 +245,22 @@ class Oracle:
         if rc:
             raise RuntimeError(f"exx_oracle_kpsi_points failed ({rc})")
         return out
+
+
+def poisson_direct_mixed(dims, spacing, periodic, table, rho):
+    """Mixed boundary conditions by the O(M^2) definition (exx_oracle_poisson_direct_mixed): periodic[a] truthy = axis a
+    is periodic (the table holds one full period there), else isolated."""
+    dims = tuple(int(d) for d in dims)
+    rho = _f64(rho).reshape(dims)
+    table = _f64(table).reshape(dims)
+    v = np.empty(dims)
+    d = np.asarray(dims, dtype=np.int32)
+    h = np.asarray(spacing, dtype=np.float64)
+    per = np.asarray([1 if x else 0 for x in periodic], dtype=np.int32)
+    rc = _load().exx_oracle_poisson_direct_mixed(d.ctypes.data_as(_ip), _d(h), per.ctypes.data_as(_ip), _d(table), _d(rho), _d(v))
+    if rc:
+        raise RuntimeError("exx_oracle_poisson_direct_mixed failed")
+    return v
 
 
 def threads_used() -> int:

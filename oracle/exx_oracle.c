@@ -766,6 +766,38 @@ int exx_oracle_poisson_direct(const exx_oracle *o, const double *rho, double *v)
     return 0;
 }
 
+/* Mixed boundary conditions (slab / wire, "free, wire, slab and periodic"), the plain definition:
+ *   V(r) = dV * sum_{r'} g(d(r, r')) rho(r'),   d_a = (r_a - r'_a) mod n_a  on a periodic axis (displacement to the
+ *   nearest-or-any image: g holds one full period there), d_a = |r_a - r'_a| on an isolated axis (g even).
+ * O(M^2) double loop, no FFT, no handle: everything is an argument.  DESIGN.md reading A24. */
+int exx_oracle_poisson_direct_mixed(const int dims[3], const double spacing[3], const int periodic[3],
+                                    const double *table, const double *rho, double *v)
+{
+    if (!dims || !spacing || !periodic || !table || !rho || !v) return 1;
+    const int n0 = dims[0], n1 = dims[1], n2 = dims[2];
+    if (n0 < 1 || n1 < 1 || n2 < 1) return 1;
+    const double dV = spacing[0] * spacing[1] * spacing[2];
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int a = 0; a < n0; ++a)
+        for (int b = 0; b < n1; ++b)
+            for (int c = 0; c < n2; ++c) {
+                ksum k = { 0.0, 0.0 };
+                for (int a2 = 0; a2 < n0; ++a2) {
+                    const int da = periodic[0] ? ((a - a2) % n0 + n0) % n0 : (a >= a2 ? a - a2 : a2 - a);
+                    for (int b2 = 0; b2 < n1; ++b2) {
+                        const int db = periodic[1] ? ((b - b2) % n1 + n1) % n1 : (b >= b2 ? b - b2 : b2 - b);
+                        for (int c2 = 0; c2 < n2; ++c2) {
+                            const int dc = periodic[2] ? ((c - c2) % n2 + n2) % n2 : (c >= c2 ? c - c2 : c2 - c);
+                            ksum_add(&k, table[((long long)da * n1 + db) * n2 + dc] *
+                                         rho[((long long)a2 * n1 + b2) * n2 + c2]);
+                        }
+                    }
+                }
+                v[((long long)a * n1 + b) * n2 + c] = dV * ksum_get(&k);
+            }
+    return 0;
+}
+
 int exx_oracle_kpsi_points(const exx_oracle *o, int n_orb, const double *psi, const double *occ,
                            int n_samples, const int *orb, const long long *point, double *out)
 {

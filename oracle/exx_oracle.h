@@ -19,7 +19,9 @@
  * P7 symmetry invariants; P8 energy/operator consistency incl. finite differences; P9 N=1 Hartree, index-n plane;
  * P10 Table 1 pair counts; P11 apply_to (coincident sets, two-cosine closed form, linearity, symmetry); P12 apply_block
  * (union of two sets = parts + block); P13 masked apply (all-ones mask, block-diagonal mask = independent subsystems);
- * P14 periodic filter table (Coulomb table = analytic kernel, screened plane-wave closed form).  Parity unpinned: none.
+ * P14 periodic filter table (Coulomb table = analytic kernel, screened plane-wave closed form); P15 mixed boundary
+ * conditions (direct sum with wrap-around = the FREE path with a periodic-even table; all axes periodic = the periodic
+ * solver).  Parity unpinned: none.
  *
  * All pointers are HOST pointers.  Arrays are C order, psi[i][a][b][c], last index fastest.
  * Return value: 0 on success, non-zero on invalid arguments / allocation failure.
@@ -92,6 +94,14 @@ int exx_oracle_realspace_kernel(const exx_oracle *o, double *g_out);
 
 /* Brute force, no FFT in the convolution: V(r) = sum_r' g(r - r') rho(r') by the O(M^2) double loop. */
 int exx_oracle_poisson_direct(const exx_oracle *o, const double *rho, double *v);
+
+/* Mixed boundary conditions (slab: two periodic axes, wire: one), the definition as an O(M^2) double loop
+ * with no FFT and no handle: V(r) = dV sum_r' g(d(r,r')) rho(r'), d_a = (r_a - r'_a) mod n_a on a periodic axis (the
+ * table holds one full period of the Green's function there), |r_a - r'_a| on an isolated one.  periodic[a] != 0 marks
+ * a periodic axis.  The claim the product relies on -- a FREE plan given a table that is even under d -> n - d along the
+ * periodic axes computes exactly this -- is pinned in tests/test_oracle_pins_ext.py (P15). */
+int exx_oracle_poisson_direct_mixed(const int dims[3], const double spacing[3], const int periodic[3],
+                                    const double *table, const double *rho, double *v);
 
 /* Sampled entries of K psi by direct real-space summation, O(N*M) each:
  * out[s] = - sum_j f_j psi_j(r_s) sum_r' g(r_s - r') psi_i(r') psi_j(r'),  i = orb[s], r_s = flat index point[s]. */

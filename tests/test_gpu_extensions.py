@@ -3,6 +3,7 @@ tests/test_oracle_pins_ext.py.  Tolerances as in test_gpu_parity.py (north_star)
 
   exx_apply_to      K of the occupied set applied to another orbital set        (NEXT-1)
   periodic filter   host-supplied Fourier-space table (screened kernel)          (NEXT-2)
+  slab / wire BC    FREE plan + one period of the mixed Green's function as data (NEXT-2)
   exx_apply_block   all pairs between two disjoint blocks + round-robin schedule (NEXT-3)
   exx_apply_pairs   sparse pair list for localised orbitals                      (NEXT-4)
 """
@@ -90,6 +91,51 @@ def test_periodic_filter_table_matches_oracle_and_closed_form(dims):
     assert abs(e2[0, 1] - khat(k) / vol) <= 1e-12 * khat(k) / vol
     assert abs(e2[0, 0] - k0 / vol) <= 1e-12 * k0 / vol
     assert abs(e2[1, 1] - (khat(2 * k) / (2 * vol) + k0 / vol)) <= 1e-12 * k0 / vol
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ NEXT-2: slab / wire boundary conditions
+@pytest.mark.parametrize("dims,periodic,n_orb", [((8, 16, 8), (1, 1, 0), 3), ((8, 8, 16), (0, 0, 1), 3)])
+def test_slab_and_wire_match_the_direct_mixed_definition(dims, periodic, n_orb):
+    """Slab (two periodic axes) and wire (one) boundary conditions are a FREE plan whose host table holds one period of
+    the mixed Green's function along the periodic axes (A24).  Reference: the oracle's O(M^2)
+    wrap-around direct sum, pair by pair (P15), combined by Eq. 3 / Eq. 5 in numpy."""
+    from oracle import poisson_direct_mixed
+    from workloads import mixed_bc_kernel_table
+    spacing = (0.45, 0.4, 0.5)
+    w = make_workload(small_spec("C2", dims=dims, n_orb=n_orb, spacing=spacing, number=700 + sum(dims)))
+    spec = w["spec"]
+    table = mixed_bc_kernel_table(dims, spacing, periodic, mu=1.2)
+    occ = np.array([2.0, 1.1, 0.4][:n_orb])
+    psi = w["psi"].numpy()
+    k_ref = np.zeros_like(psi)
+    ex_ref = 0.0
+    for i in range(n_orb):
+        for j in range(n_orb):
+            v = poisson_direct_mixed(dims, spacing, periodic, table, psi[i] * psi[j])
+            k_ref[i] -= occ[j] * v * psi[j]
+            ex_ref -= 0.5 * occ[i] * occ[j] * spec.dV * float(np.sum(psi[i] * psi[j] * v))
+    plan = exx.ExxPlan(spec.dims, spec.spacing, "free", table, max_orbitals=n_orb)
+    kpsi, ex = plan.apply(w["psi"].cuda(), occ)
+    assert np.max(np.abs(kpsi.cpu().numpy() - k_ref)) <= K_RTOL * np.max(np.abs(k_ref))
+    assert abs(ex - ex_ref) <= E_RTOL * abs(ex_ref)
+    plan.destroy()
+
+
+def test_slab_at_a_warp_specialised_size_matches_the_oracle():
+    """The same at 48 x 48 x 24 (transform grid 96 x 96 x 48) against the oracle's FFT path with the same table -- which
+    P15 ties to the wrap-around definition."""
+    from workloads import mixed_bc_kernel_table
+    dims, n_orb = (48, 48, 24), 4
+    w = make_workload(small_spec("C2", dims=dims, n_orb=n_orb, spacing=(0.45, 0.4, 0.5), number=777))
+    spec = w["spec"]
+    table = mixed_bc_kernel_table(dims, spec.spacing, (1, 1, 0), mu=0.8)
+    occ = np.array([2.0, 1.0, 0.0, 1.5])
+    plan = exx.ExxPlan(spec.dims, spec.spacing, "free", table, max_orbitals=n_orb)
+    kpsi, ex = plan.apply(w["psi"].cuda(), occ)
+    k_ref, ex_ref, _ = Oracle(spec.dims, spec.spacing, "free", table).apply(w["psi"].numpy(), occ)
+    assert np.max(np.abs(kpsi.cpu().numpy() - k_ref)) <= K_RTOL * np.max(np.abs(k_ref))
+    assert abs(ex - ex_ref) <= E_RTOL * abs(ex_ref)
     plan.destroy()
 
 

@@ -175,3 +175,73 @@ def test_p14_screened_plane_wave_closed_form():
     kk = k @ k
     v = o.poisson(rho)
     assert np.max(np.abs(v - 4 * np.pi / kk * (1 - np.exp(-kk / (4 * omega ** 2))) * rho)) <= 1e-13 * (4 * np.pi / kk)
+
+
+# ------------------------------------------------------------------------------------------------ P15 mixed BC (slab / wire)
+def _even_table(rng, dims, periodic):
+    """Random positive table, made even under index -> n - index along the periodic axes (what a Green's function is)."""
+    g = rng.random(dims) + 0.1
+    for ax in range(3):
+        if periodic[ax]:
+            g = 0.5 * (g + np.take(g, (-np.arange(dims[ax])) % dims[ax], axis=ax))
+    return g
+
+
+@pytest.mark.parametrize("dims,periodic", [((4, 6, 3), (1, 1, 0)), ((3, 4, 6), (0, 0, 1)), ((4, 3, 5), (1, 0, 1)), ((3, 4, 4), (0, 0, 0))])
+def test_p15_point_charge_reads_the_table_with_wrap(dims, periodic):
+    """A unit point charge at r0 gives V(r) = dV g(d(r, r0)): periodic axes wrap (roll), isolated axes take |r - r0|."""
+    from oracle import poisson_direct_mixed
+    rng = np.random.default_rng(1501)
+    spacing = (0.5, 0.4, 0.3)
+    g = _even_table(rng, dims, periodic)
+    r0 = (dims[0] - 1, 1, dims[2] // 2)
+    rho = np.zeros(dims)
+    rho[r0] = 1.0
+    got = poisson_direct_mixed(dims, spacing, periodic, g, rho)
+    want = g
+    for ax in range(3):
+        n = dims[ax]
+        idx = (np.arange(n) - r0[ax]) % n if periodic[ax] else np.abs(np.arange(n) - r0[ax])
+        want = np.take(want, idx, axis=ax)
+    want = want * np.prod(spacing)
+    assert np.max(np.abs(got - want)) <= 1e-15 * np.max(np.abs(want))
+
+
+@pytest.mark.parametrize("dims,periodic", [((4, 6, 3), (1, 1, 0)), ((3, 4, 6), (0, 0, 1)), ((4, 4, 4), (1, 1, 1))])
+def test_p15_free_path_with_a_periodic_even_table_is_the_mixed_solver(dims, periodic):
+    """The claim behind slab / wire support (A24): zero-padded (Hockney) convolution with table[|d|] equals the
+    wrap-around convolution along every axis on which the table is even under d -> n - d."""
+    from oracle import poisson_direct_mixed
+    rng = np.random.default_rng(1502)
+    spacing = (0.5, 0.4, 0.3)
+    g = _even_table(rng, dims, periodic)
+    rho = rng.standard_normal(dims)
+    want = poisson_direct_mixed(dims, spacing, periodic, g, rho)
+    got = Oracle(dims, spacing, "free", g).poisson(rho)
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+def test_p15_all_axes_periodic_reproduces_the_periodic_solver():
+    """With the real-space image of 4 pi/|G|^2 as the table, the mixed solver with three periodic axes -- by the direct
+    sum and through the FREE path -- is the (pinned: P3, P4) periodic Poisson solver."""
+    from oracle import poisson_direct_mixed
+    dims, spacing = (4, 6, 4), (0.5, 0.4, 0.45)
+    o = Oracle(dims, spacing, "periodic")
+    table = o.realspace_kernel() / np.prod(spacing)
+    rng = np.random.default_rng(1503)
+    rho = rng.standard_normal(dims)
+    want = o.poisson(rho)
+    got_direct = poisson_direct_mixed(dims, spacing, (1, 1, 1), table, rho)
+    got_free = Oracle(dims, spacing, "free", table).poisson(rho)
+    scale = np.max(np.abs(want))
+    assert np.max(np.abs(got_direct - want)) <= 1e-12 * scale
+    assert np.max(np.abs(got_free - want)) <= 1e-12 * scale
+
+
+def test_p15_screened_image_table_is_even_and_decays():
+    from workloads import mixed_bc_kernel_table
+    dims, spacing = (8, 6, 8), (0.5, 0.6, 0.5)
+    g = mixed_bc_kernel_table(dims, spacing, (1, 0, 1), mu=2.0)
+    for ax in (0, 2):
+        assert np.array_equal(g, np.take(g, (-np.arange(dims[ax])) % dims[ax], axis=ax))
+    assert g[0, 0, 0] > g[1, 0, 0] > g[2, 0, 0] > 0 and g[0, 5, 0] < 1e-3 * g[0, 1, 0]

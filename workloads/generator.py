@@ -210,6 +210,45 @@ def free_kernel_table(dims, spacing) -> np.ndarray:
     return np.ascontiguousarray(g)
 
 
+def mixed_bc_kernel_table(dims, spacing, periodic, mu: float, images: int = 2) -> np.ndarray:
+    """Host table for slab / wire boundary conditions, handed to a FREE-BC plan as data: the short-range
+    screened Coulomb kernel erfc(mu r)/r (the HSE-type filter of PAPER.md:236 in real space) summed over the periodic
+    images along the axes marked periodic,
+        g[a][b][c] = sum_{m} erfc(mu |d + m L|) / |d + m L|,   d = (a h1, b h2, c h3),  m_axis = -images..images,
+    where L_axis = n_axis h_axis on periodic axes and m_axis = 0 on isolated ones.  Along a periodic axis the table holds
+    one full period and is even under index -> n - index (up to the truncated image sum, which erfc makes negligible
+    for mu L >= 4); the d = 0 entry takes the cell average of 1/r minus the r -> 0 limit 2 mu / sqrt(pi) of
+    (1 - erfc)/r.  Input data only: none of the method's arithmetic."""
+    from math import erfc, pi, sqrt
+    n = [int(d) for d in dims]
+    h = [float(x) for x in spacing]
+    per = [bool(x) for x in periodic]
+    rng = [range(-images, images + 1) if per[ax] else range(0, 1) for ax in range(3)]
+    ax_d = [np.arange(n[ax]) * h[ax] for ax in range(3)]
+    verfc = np.vectorize(erfc)
+    g = np.zeros(n, dtype=np.float64)
+    for m0 in rng[0]:
+        for m1 in rng[1]:
+            for m2 in rng[2]:
+                x = (ax_d[0] + m0 * n[0] * h[0])[:, None, None]
+                y = (ax_d[1] + m1 * n[1] * h[1])[None, :, None]
+                z = (ax_d[2] + m2 * n[2] * h[2])[None, None, :]
+                r = np.sqrt(x * x + y * y + z * z)
+                home = m0 == 0 and m1 == 0 and m2 == 0
+                if home:
+                    r[0, 0, 0] = 1.0
+                term = verfc(mu * r) / r
+                if home:
+                    term[0, 0, 0] = cell_average_inverse_r(h) - 2.0 * mu / sqrt(pi)
+                g += term
+    # make the evenness along periodic axes exact (the truncated image sum breaks it at the 1e-16..1e-12 level)
+    for ax in range(3):
+        if per[ax]:
+            idx = (-np.arange(n[ax])) % n[ax]
+            g = 0.5 * (g + np.take(g, idx, axis=ax))
+    return np.ascontiguousarray(g)
+
+
 def make_workload(spec_or_name, device="cpu") -> dict:
     """Orbitals, occupations and (free BC) the Green's-function table for a config name or a WorkloadSpec."""
     spec = CONFIGS[spec_or_name] if isinstance(spec_or_name, str) else spec_or_name
