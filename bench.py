@@ -459,6 +459,7 @@ def run_ours(args, rank, local_rank, world):
         dist.destroy_process_group()
         return
     fp64 = exx.exx_diag_fp64(torch.cuda.current_stream().cuda_stream)
+    fp64.update(exx.exx_diag_shfl(torch.cuda.current_stream().cuda_stream))
 
     # ---- the other target configurations, same run, device-resident only
     per_config = {}

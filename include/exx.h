@@ -230,6 +230,14 @@ exx_status exx_plan_set_batch(exx_plan *plan, int max_transforms_per_batch);
  */
 exx_status exx_diag_fp64(void *cuda_stream, double *dfma_tflops, double *dadd_tops, double *lds_gbs, double *overlap_ratio);
 
+/*
+ * exx_diag_shfl -- companion microbenchmark: bandwidth of 32-bit warp shuffles (GB/s summed over the SMs, 4 bytes per lane
+ * per SHFL) and how far shuffles issued by some warps overlap with 16-byte shared-memory loads issued by others (1 = the
+ * two add up, 0 = they share one datapath).  It is the measurement behind exchanging the FFT stages through shared memory
+ * rather than through warp shuffles.  Diagnostic only.  Synchronises.
+ */
+exx_status exx_diag_shfl(void *cuda_stream, double *shfl_gbs, double *shfl_lds_overlap);
+
 exx_status  exx_plan_destroy(exx_plan *plan);       /* NULL is allowed */
 const char *exx_status_string(exx_status s);
 const char *exx_last_error(const exx_plan *plan);   /* detail text incl. CUDA error name; plan may be NULL for

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     ExxPlan,
     exx_apply,
     exx_diag_fp64,
+    exx_diag_shfl,
     exx_plan_create,
     exx_plan_destroy,
     exx_round_robin_step,

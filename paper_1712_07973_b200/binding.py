@@ -27,7 +27,7 @@ EXPORTS = [
     "exx_get_pair_energies", "exx_get_block_energies", "exx_plan_release_staging",
     "exx_schedule_pairs", "exx_schedule_list", "exx_schedule_list_masked", "exx_schedule_list_block", "exx_round_robin_step",
     "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_device", "exx_plan_kernel_name",
-    "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version", "exx_diag_fp64",
+    "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version", "exx_diag_fp64", "exx_diag_shfl",
 ]
 
 _lib = None
@@ -107,6 +107,8 @@ def load_library():
     lib.exx_last_error.restype = C.c_char_p
     lib.exx_diag_fp64.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
     lib.exx_diag_fp64.restype = C.c_int
+    lib.exx_diag_shfl.argtypes = [C.c_void_p, _dp, _dp]
+    lib.exx_diag_shfl.restype = C.c_int
     lib.exx_version.argtypes = []
     lib.exx_version.restype = C.c_char_p
     _lib = lib
@@ -124,6 +126,15 @@ def exx_diag_fp64(stream: Optional[int] = None) -> dict:
     if st:
         raise ExxError(st, "exx_diag_fp64")
     return {"dfma_tflops": v[0].value, "dadd_tera_inst_per_s": v[1].value, "lds_gbs": v[2].value, "fp64_lds_overlap": v[3].value}
+
+
+def exx_diag_shfl(stream: Optional[int] = None) -> dict:
+    """Measured warp-shuffle bandwidth and its overlap with shared-memory loads (include/exx.h exx_diag_shfl)."""
+    v = [C.c_double() for _ in range(2)]
+    st = load_library().exx_diag_shfl(C.c_void_p(stream) if stream else None, *[C.byref(x) for x in v])
+    if st:
+        raise ExxError(st, "exx_diag_shfl")
+    return {"shfl_gbs": v[0].value, "shfl_lds_overlap": v[1].value}
 
 
 def exx_schedule_pairs(occ: Sequence[float]):

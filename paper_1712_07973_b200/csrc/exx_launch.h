@@ -139,7 +139,12 @@ struct TuneAC {
     // ---- pass C
     static constexpr int G_C = pick_g<TC, TB, FREE>(true, kMaxSmemAC / 2);
     using CfgC = CfgAC<TC, TB, FREE, G_C, CHUNK>;
-    static constexpr int NT_C = imax(32, round_up32(imax(CfgC::ITEMS_LINE_Q, imin(CfgC::ITEMS_POS, 256))));
+    // threads: one per (line, n2) item of C2 and, where that is fewer than the columns of C0 (free BC: the tile has twice as
+    // many columns as C2 items), still only that many once they are >= 128 -- the warps that would idle through C1 / C2
+    // are dropped, each thread takes two columns in C0, and the larger register budget admits the early gather
+    // (256^3 free: pass C -6 %)
+    static constexpr int NT_C_WIDE = imax(32, round_up32(imax(CfgC::ITEMS_LINE_Q, imin(CfgC::ITEMS_POS, 256))));
+    static constexpr int NT_C = (CfgC::ITEMS_LINE_Q >= 128 && round_up32(CfgC::ITEMS_LINE_Q) < NT_C_WIDE) ? round_up32(CfgC::ITEMS_LINE_Q) : NT_C_WIDE;
     // double-buffered W1 tile where it fits next to one operand stage and the resident lines, else single-buffered
     // W1 tile buffers (NBUF) and operand stages (NSTG): the deepest pipeline with which two CTAs share an SM (the other
     // CTA then covers what a shallower pipeline exposes), else the deepest one that fits at all

@@ -150,6 +150,42 @@ def test_warp_specialised_kernels_edge_schedule(base, dims):
     assert abs(ex_a - ex_b) <= 1e-13 * abs(ex_a) and abs(ex_a - ex_c) <= 1e-13 * abs(ex_a)
 
 
+@pytest.mark.parametrize("base,dims,n_orb,batch", [("C1", (32, 32, 32), 5, 2), ("C1", (96, 96, 96), 5, 3), ("C2", (48, 48, 48), 4, 0),
+                                                   ("C1", (192, 96, 48), 3, 2), ("C2", (16, 64, 32), 3, 0)])
+def test_guard_bands_and_poisoned_outputs(base, dims, n_orb, batch):
+    """Memory-safety evidence that needs no tool (compute-sanitizer is closed on this pool): psi and K psi live in the
+    middle of larger allocations whose guard bands hold a sentinel, K psi starts as NaN, and E_x / e_ij start as NaN.
+    After the apply the guard bands and psi must be bit-for-bit what they were (no stray store, no stray reduce-add:
+    an add onto the sentinel would change it), and the outputs must be finite everywhere and equal to those of a plain
+    run (every output element was written, nothing read an output before writing it)."""
+    w = make_workload(small_spec(base, dims=dims, n_orb=n_orb, number=1300 + sum(dims)))
+    spec = w["spec"]
+    m = spec.n_orb * spec.n_points
+    guard = 1 << 16
+    sentinel = 1.2345678901234567e+100
+    buf_p = torch.full((m + 2 * guard,), sentinel, dtype=torch.float64, device="cuda")
+    buf_k = torch.full((m + 2 * guard,), sentinel, dtype=torch.float64, device="cuda")
+    psi = buf_p[guard:guard + m].view(spec.n_orb, *spec.dims)
+    kpsi = buf_k[guard:guard + m].view(spec.n_orb, *spec.dims)
+    psi.copy_(w["psi"].cuda())
+    psi_before = psi.clone()
+    kpsi.fill_(float("nan"))
+    ex_dev = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+    plan = exx.ExxPlan(spec.dims, spec.spacing, spec.bc, w["kernel"], max_orbitals=spec.n_orb)
+    if batch:
+        plan.set_batch(batch)
+    occ = np.array([2.0, 1.0, 0.0, 0.5, 1.5][:n_orb])
+    plan.apply_async(psi, occ, kpsi, ex_dev)
+    torch.cuda.synchronize()
+    for buf in (buf_p, buf_k):
+        assert bool((buf[:guard] == sentinel).all()) and bool((buf[guard + m:] == sentinel).all())
+    assert torch.equal(psi, psi_before)
+    assert bool(torch.isfinite(kpsi).all()) and bool(torch.isfinite(ex_dev).all())
+    k_plain, ex_plain = plan.apply(w["psi"].cuda(), occ)
+    assert torch.equal(kpsi, k_plain) and float(ex_dev[0]) == ex_plain
+    plan.destroy()
+
+
 def test_pointer_and_argument_errors():
     w = make_workload(small_spec("C1", dims=(16, 16, 16), n_orb=2, number=79))
     plan = exx.ExxPlan((16, 16, 16), w["spec"].spacing, "periodic", None, max_orbitals=2)
