@@ -1184,6 +1184,15 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     }
 
     XformDesc d_next = g.desc[0];                              // descriptor of the next transform, one iteration ahead
+    // The operand stage of transform t is refilled (for t + NSTG) by warp 0 once the reduce-adds of t have READ it.  Waiting
+    // for that right after issuing them would idle warp 0 while the other warps already run C0 of t+1 and then wait for it
+    // at the next barrier; instead the refill is deferred to after warp 0's own C0 of t+1, when the reads are long done.
+#ifdef EXX_C_REFILL_EAGER
+    constexpr bool DEFER = false;
+#else
+    constexpr bool DEFER = true;
+#endif
+    int refill_t = -1, refill_s = 0;
     for (int t = 0; t < g.count; ++t) {
         double2* S = S0 + (NBUF == 2 ? (t & 1) : 0) * C::SMEM_C;
         const int s = t % NSTG;
@@ -1204,6 +1213,12 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
             if (tid + m * NT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, s_twb + c0[m].b2 * C::R1);
+        if (DEFER && tid < 32 && refill_t >= 0) {
+            bulk_wait_read_all();                          // the stage may be overwritten
+            __syncwarp();
+            issue_operand_loads<C>(g, g.desc[refill_t], OP + static_cast<size_t>(refill_s) * C::OP_DOUBLES, &full[refill_s], a, b2base, tid);
+            refill_t = -1;
+        }
         __syncthreads();
 #pragma unroll
         for (int m = 0; m < NI1; ++m)
@@ -1246,7 +1261,7 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         }
         if ((tid & 31) == 0) { red[0][tid >> 5] = e1; red[1][tid >> 5] = e2; }
         __syncthreads();                                   // also: S and the operand stage are no longer read
-        if (tid == 0) {
+        if (tid == NT - 32) {                              // first lane of the last warp: warp 0 has the TMA traffic to issue
             double s1 = 0.0, s2 = 0.0;
 #pragma unroll
             for (int k = 0; k < NT / 32; ++k) { s1 += red[0][k]; s2 += red[1][k]; }
@@ -1262,9 +1277,13 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             }
             bulk_commit();
             if (t + NSTG < g.count) {
-                bulk_wait_read_all();                      // the stage may be overwritten
-                __syncwarp();
-                issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+                if (DEFER) {
+                    refill_t = t + NSTG; refill_s = s;
+                } else {
+                    bulk_wait_read_all();                  // the stage may be overwritten
+                    __syncwarp();
+                    issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+                }
             }
         }
     }
