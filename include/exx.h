@@ -80,6 +80,20 @@ exx_status exx_plan_create(exx_plan **plan, const int dims[3], const double spac
                            const double *kernel_host, int max_orbitals, void *cuda_stream);
 
 /*
+ * exx_plan_create_general -- periodic cell of ANY shape (non-orthorhombic lattice vectors a1, a2, a3; the
+ * solver is "completely general").  The grid points are r = (i1/n1) a1 + (i2/n2) a2 + (i3/n3) a3, so the transforms are the
+ * same as for an orthorhombic cell; what differs is the Fourier-space kernel, which is no longer even in every index:
+ *   khat_full_host  HOST, K^[m1][m2][m3], n1*n2*n3 doubles on the FULL FFT index grid (index m_a <-> frequency m_a for
+ *                   m_a <= n_a/2, m_a - n_a above), e.g. 4 pi / |m1 b1 + m2 b2 + m3 b3|^2 with the reciprocal vectors b_a
+ *                   and K^(0) = 0; must satisfy K^(-m) = K^(m) for real potentials; WITHOUT the 1/(n1 n2 n3) of the inverse
+ *                   transform.  Copied during the call.
+ *   cell_volume     |a1 . (a2 x a3)| in bohr^3: only dV = cell_volume / (n1 n2 n3) enters (energies, A10).
+ * dims, max_orbitals, cuda_stream as exx_plan_create.  DESIGN.md reading A25.
+ */
+exx_status exx_plan_create_general(exx_plan **plan, const int dims[3], double cell_volume, const double *khat_full_host,
+                                   int max_orbitals, void *cuda_stream);
+
+/*
  * exx_apply -- the hot path: K psi for all orbitals and E_x (PAPER.md:67-69 Eq. 3, :81-82 Eq. 5).
  *   psi_dev   DEVICE, [n_orb][n1][n2][n3] doubles, contiguous, read-only, 16-byte aligned.
  *   occ_host  HOST, [n_orb] occupations f_i.  A pair with f_i = f_j = 0 is skipped.

@@ -40,6 +40,7 @@ def _load():
         lib.exx_oracle_apply_to.argtypes = [C.c_void_p, C.c_int, _dp, _dp, C.c_int, _dp, _dp]
         lib.exx_oracle_apply_block.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp]
         lib.exx_oracle_set_periodic_filter.argtypes = [C.c_void_p, _dp]
+        lib.exx_oracle_set_periodic_filter_full.argtypes = [C.c_void_p, _dp]
         lib.exx_oracle_poisson_direct_mixed.argtypes = [_ip, _dp, _ip, _dp, _dp, _dp]
         lib.exx_oracle_threads.argtypes = []
         _lib = lib
@@ -97,6 +98,19 @@ class Oracle:
         t = (C.c_int * 3)()
         lib.exx_oracle_transform_dims(self._h, t)
         self.tdims = tuple(t)
+
+    @classmethod
+    def general(cls, dims, cell_volume, khat_full):
+        """Periodic cell of any shape: khat_full = K^ on the full FFT index grid [n1][n2][n3]; dV = cell_volume / M."""
+        dims = tuple(int(d) for d in dims)
+        h = (float(cell_volume) / (dims[0] * dims[1] * dims[2])) ** (1.0 / 3.0)
+        o = cls(dims, (h, h, h), "periodic")
+        t = _f64(khat_full)
+        if t.shape != dims:
+            raise ValueError("khat_full must have shape dims")
+        if _load().exx_oracle_set_periodic_filter_full(o._h, _d(t)):
+            raise RuntimeError("exx_oracle_set_periodic_filter_full failed")
+        return o
 
     def close(self):
         if self._h:

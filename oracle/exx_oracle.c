@@ -258,6 +258,17 @@ int exx_oracle_set_periodic_filter(exx_oracle *o, const double *table)
     return 0;
 }
 
+/* General periodic cell (non-orthorhombic lattice; reading A25): K^ given on the FULL transform grid, used as is. */
+int exx_oracle_set_periodic_filter_full(exx_oracle *o, const double *table_full)
+{
+    if (!o || !table_full || o->bc != EXX_ORACLE_PERIODIC) return 1;
+    for (long long x = 0; x < o->T; ++x) {
+        o->khat[x].re = table_full[x];
+        o->khat[x].im = 0.0;
+    }
+    return 0;
+}
+
 void exx_oracle_destroy(exx_oracle *o)
 {
     if (!o) return;

@@ -21,7 +21,8 @@
  * (union of two sets = parts + block); P13 masked apply (all-ones mask, block-diagonal mask = independent subsystems);
  * P14 periodic filter table (Coulomb table = analytic kernel, screened plane-wave closed form); P15 mixed boundary
  * conditions (direct sum with wrap-around = the FREE path with a periodic-even table; all axes periodic = the periodic
- * solver).  Parity unpinned: none.
+ * solver); P16 general periodic cells (full-grid filter = the folded filter for an even table; triclinic plane-wave closed
+ * form; brute-force convolution with the real-space image of the table).  Parity unpinned: none.
  *
  * All pointers are HOST pointers.  Arrays are C order, psi[i][a][b][c], last index fastest.
  * Return value: 0 on success, non-zero on invalid arguments / allocation failure.
@@ -79,6 +80,10 @@ int exx_oracle_apply_block(const exx_oracle *o, int n_a, const double *psi_a, co
 /* PERIODIC only: use the host table K^[s0][s1][s2] (symmetric index range s = 0..t/2 per axis, even in every index)
  * instead of 4 pi/|G|^2 (screened hybrids change only this filter). */
 int exx_oracle_set_periodic_filter(exx_oracle *o, const double *table);
+
+/* PERIODIC only, general (non-orthorhombic) cells: K^[m0][m1][m2] on the FULL transform grid (FFT index order), used as
+ * is; dV is the product of the spacings given at creation (pass three equal nominal spacings cbrt(cell volume / M)). */
+int exx_oracle_set_periodic_filter_full(exx_oracle *o, const double *table_full);
 
 /* Complete rows: for each listed i, Kpsi_i (all j) into kpsi_rows[row][M] and e_ij into e_rows[row][N] (may be NULL). */
 int exx_oracle_rows(const exx_oracle *o, int n_orb, const double *psi, const double *occ,

@@ -23,7 +23,7 @@ _STATUS = ["EXX_OK", "EXX_ERR_INVALID_ARG", "EXX_ERR_UNSUPPORTED_SIZE", "EXX_ERR
 EXX_BLOCK_ACCUMULATE_RESIDENT, EXX_BLOCK_ACCUMULATE_STREAMED = 1, 2
 
 EXPORTS = [
-    "exx_plan_create", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_apply_pairs", "exx_apply_to", "exx_apply_block",
+    "exx_plan_create", "exx_plan_create_general", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_apply_pairs", "exx_apply_to", "exx_apply_block",
     "exx_get_pair_energies", "exx_get_block_energies", "exx_plan_release_staging",
     "exx_schedule_pairs", "exx_schedule_list", "exx_schedule_list_masked", "exx_schedule_list_block", "exx_round_robin_step",
     "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_device", "exx_plan_kernel_name",
@@ -56,6 +56,8 @@ def load_library():
     lib = C.CDLL(path)
     lib.exx_plan_create.argtypes = [C.POINTER(C.c_void_p), _ip, _dp, C.c_int, _dp, C.c_int, C.c_void_p]
     lib.exx_plan_create.restype = C.c_int
+    lib.exx_plan_create_general.argtypes = [C.POINTER(C.c_void_p), _ip, C.c_double, _dp, C.c_int, C.c_void_p]
+    lib.exx_plan_create_general.restype = C.c_int
     for name in ("exx_apply", "exx_apply_async", "exx_apply_host"):
         fn = getattr(lib, name)
         fn.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_void_p]
@@ -229,6 +231,26 @@ class ExxPlan:
                                  C.c_void_p(stream) if stream else None)
         if st:
             raise ExxError(st, lib.exx_last_error(None).decode())
+
+    @classmethod
+    def general(cls, dims, cell_volume, khat_full, max_orbitals=1, stream: Optional[int] = None):
+        """Periodic cell of any shape (exx_plan_create_general): khat_full = K^[m1][m2][m3] on the full FFT index grid."""
+        lib = load_library()
+        self = cls.__new__(cls)
+        self.dims = tuple(int(d) for d in dims)
+        self.bc = EXX_BC_PERIODIC
+        self.max_orbitals = int(max_orbitals)
+        h = (float(cell_volume) / (self.dims[0] * self.dims[1] * self.dims[2])) ** (1.0 / 3.0)
+        self.spacing = (h, h, h)
+        self._kernel = np.ascontiguousarray(np.asarray(khat_full, dtype=np.float64))
+        if self._kernel.shape != self.dims:
+            raise ValueError(f"khat_full must have shape {self.dims}")
+        self._h = C.c_void_p()
+        st = lib.exx_plan_create_general(C.byref(self._h), (C.c_int * 3)(*self.dims), C.c_double(float(cell_volume)),
+                                         self._kernel.ctypes.data_as(_dp), self.max_orbitals, C.c_void_p(stream) if stream else None)
+        if st:
+            raise ExxError(st, lib.exx_last_error(None).decode())
+        return self
 
     # -- helpers
     def _check(self, st):

@@ -100,6 +100,20 @@ __global__ void permute_kernel_axes(const double* ks_sym, double* ks_perm, int n
     }
 }
 
+// General periodic cells: ks_perm[kb][p][ka] = scale * table[ka][kb][kc(p)], every frequency index along a and b, the c
+// index in the digit-scrambled order of the in-tile FFT (position p = k1*QC + k2 holds frequency kc = k1 + PC*k2).
+__global__ void permute_full_kernel(const double* table, double* ks_perm, int ta, int tb, int tc, int pc, int qc, double scale) {
+    const long long total = static_cast<long long>(tb) * tc * ta;
+    for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
+         x += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int ka = static_cast<int>(x % ta);
+        const int p = static_cast<int>((x / ta) % tc);
+        const int kb = static_cast<int>(x / (static_cast<long long>(ta) * tc));
+        const int kc = (p / qc) + pc * (p % qc);
+        ks_perm[x] = scale * table[(static_cast<long long>(ka) * tb + kb) * tc + kc];
+    }
+}
+
 // ks[x] *= scale  (host-supplied periodic Fourier table: fold in the 1/T_tot of the inverse transform)
 __global__ void scale_kernel(double* ks, long long total, double scale) {
     for (long long x = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; x < total;
@@ -198,6 +212,7 @@ struct exx_plan {
     int last_rows, last_cols;   // shape of the energy matrix the most recent apply left in e_mat (0: none)
     int last_rect;          // 1: that matrix is a rectangular block [n_res][n_str], 0: the symmetric [n][n] one
     int custom_kernel;      // periodic BC with a host-supplied Fourier table
+    int fullk;              // that table covers every frequency index (general cell, exx_plan_create_general): ks is [TB][TC][TA]
     int profiling;
     std::vector<cudaEvent_t> events;   // 5 per batch when profiling (pool grown by exx_plan_set_profiling / set_batch)
     size_t events_used;
@@ -331,7 +346,31 @@ int default_batch(const exx_plan* p) {
     return static_cast<int>(b);
 }
 
+// general periodic cell: the host table K^[m1][m2][m3] on the full FFT index grid, 1/T_tot folded in here
+exx_status build_full_fourier_kernel(exx_plan* p, const double* khat_full_host) {
+    const size_t total = static_cast<size_t>(p->t[0]) * p->t[1] * p->t[2];
+    double* tmp = nullptr;
+    if (cudaMalloc(&p->ks, total * sizeof(double)) != cudaSuccess || cudaMalloc(&tmp, total * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        if (tmp) cudaFree(tmp);
+        return fail(p, EXX_ERR_ALLOC, "cudaMalloc(Fourier kernel) failed");
+    }
+    int pc = 0, qc = 0;
+    split_of(p->t[2], &pc, &qc);
+    cudaError_t e = cudaMemcpyAsync(tmp, khat_full_host, total * sizeof(double), cudaMemcpyHostToDevice, p->stream);
+    if (e == cudaSuccess) {
+        permute_full_kernel<<<4096, 256, 0, p->stream>>>(tmp, p->ks, p->t[0], p->t[1], p->t[2], pc, qc, 1.0 / static_cast<double>(total));
+        ++p->launches;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return cuda_fail(p, e, "building the full Fourier kernel");
+    return EXX_OK;
+}
+
 exx_status build_fourier_kernel(exx_plan* p, const double* kernel_host) {
+    if (p->fullk) return build_full_fourier_kernel(p, kernel_host);
     const int na = p->t[0] / 2 + 1, nb = p->t[1] / 2 + 1, nc = p->t[2] / 2 + 1;
     const size_t total = static_cast<size_t>(na) * nb * nc;
     const size_t total_perm = static_cast<size_t>(na) * nb * p->t[2];
@@ -454,7 +493,7 @@ exx_status run_job_unguarded(exx_plan* p, const Job& job) {
     ac.w1 = p->w1; ac.twc = p->tw[2]; ac.twb = p->twb; ac.epart = p->epart;
     ac.m_points = p->M; ac.na = p->n[0];
     ArgsB ab{};
-    ab.w1 = p->w1; ab.twa = p->tw[0]; ab.ks = p->ks; ab.tc = p->t[2];
+    ab.w1 = p->w1; ab.twa = p->tw[0]; ab.ks = p->ks; ab.fullk = p->fullk; ab.tc = p->t[2];
     ab.npch = p->t[2] / p->geo.chunk;
 
     p->events_used = 0;
@@ -694,8 +733,8 @@ exx_status exx_round_robin_step(int n_ranks, int rank, int step, int* send_to, i
     return EXX_OK;
 }
 
-exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spacing[3], exx_bc bc, const double* kernel_host,
-                           int max_orbitals, void* cuda_stream) {
+static exx_status create_impl(exx_plan** plan, const int dims[3], const double spacing[3], exx_bc bc, const double* kernel_host,
+                              int fullk, int max_orbitals, void* cuda_stream) {
     g_create_error.clear();
     if (!plan || !dims || !spacing) return fail(nullptr, EXX_ERR_INVALID_ARG, "NULL argument");
     *plan = nullptr;
@@ -744,6 +783,7 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     p->max_orb = max_orbitals;
     p->stream = static_cast<cudaStream_t>(cuda_stream);
     p->custom_kernel = (bc == EXX_BC_PERIODIC && kernel_host) ? 1 : 0;
+    p->fullk = fullk;
 
     auto bail = [&](exx_status st) {
         g_create_error = p->err;
@@ -815,13 +855,34 @@ exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spac
     }
     std::memset(p->occ_pinned, 0, 2 * n * sizeof(double));
     p->fixed_bytes = n * n * sizeof(double) + 2 * n * sizeof(double) + p->desc_cap * sizeof(XformDesc) +
-                     sizeof(double) * (static_cast<size_t>(p->t[0] / 2 + 1) * (p->t[1] / 2 + 1) * p->t[2]);
+                     sizeof(double) * (fullk ? static_cast<size_t>(p->t[0]) * p->t[1] * p->t[2]
+                                             : static_cast<size_t>(p->t[0] / 2 + 1) * (p->t[1] / 2 + 1) * p->t[2]);
     if (cudaMemset(p->e_mat, 0, n * n * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
         return bail(fail(p, EXX_ERR_CUDA, "cudaMemset failed"));
     }
     *plan = p;
     return EXX_OK;
+}
+
+exx_status exx_plan_create(exx_plan** plan, const int dims[3], const double spacing[3], exx_bc bc, const double* kernel_host,
+                           int max_orbitals, void* cuda_stream) {
+    return create_impl(plan, dims, spacing, bc, kernel_host, 0, max_orbitals, cuda_stream);
+}
+
+exx_status exx_plan_create_general(exx_plan** plan, const int dims[3], double cell_volume, const double* khat_full_host,
+                                   int max_orbitals, void* cuda_stream) {
+    g_create_error.clear();
+    if (!plan || !dims) return fail(nullptr, EXX_ERR_INVALID_ARG, "NULL argument");
+    *plan = nullptr;
+    if (!khat_full_host) return fail(nullptr, EXX_ERR_INVALID_ARG, "a general periodic cell needs its Fourier-space table");
+    if (!(cell_volume > 0.0) || !std::isfinite(cell_volume)) return fail(nullptr, EXX_ERR_INVALID_ARG, "cell_volume must be > 0");
+    for (int ax = 0; ax < 3; ++ax)
+        if (dims[ax] < 1) return fail(nullptr, EXX_ERR_UNSUPPORTED_SIZE, "non-positive grid length");
+    // only dV = cell_volume / (n1 n2 n3) enters the path (energies); it is carried as three equal nominal spacings
+    const double h = std::cbrt(cell_volume / (static_cast<double>(dims[0]) * dims[1] * dims[2]));
+    const double spacing[3] = {h, h, h};
+    return create_impl(plan, dims, spacing, EXX_BC_PERIODIC, khat_full_host, 1, max_orbitals, cuda_stream);
 }
 
 exx_status exx_plan_destroy(exx_plan* p) {

@@ -483,7 +483,8 @@ struct ArgsB {
     const double2* twa;         // [k1*QA + n2] = W_TA^{n2 k1}
     const double* ks;           // Fourier kernel [TB/2+1][tc][TA/2+1]: symmetric index along b, SCRAMBLED position p
                                 // along c (the order pass B meets it), symmetric index along a fastest; includes
-                                // 1/T_tot (and dV)
+                                // 1/T_tot (and dV).  fullk: [TB][tc][TA], every frequency index along a and b
+    int fullk;
     int tc;                     // c-axis transform length
     int npch;                   // tc / CHUNK
     int count;                  // transforms in the batch
@@ -550,12 +551,20 @@ EXX_HD void b1_compute(double2* colp, const double2* tw, int tws) {
 //      conj twiddle W_TA^{-n2 k1} = conj(tw[n2*tws]).
 // K^ values of one B2 item (frequencies ka = k1 + PA k2, symmetric index): issued well before they are used so that
 // the L2 latency hides behind the FFT stages in between
+// K^ comes in two layouts (ArgsB::fullk): folded -- symmetric index ranges along a and b, for kernels that are even in
+// every index (the analytic and the tabulated ones of an orthorhombic cell, every free-BC kernel) -- and full -- every
+// frequency index of a and b, for general periodic cells whose K^(m) = K^(-m) only (exx_plan_create_general).
 template <class C>
-EXX_HD void b2_load_k(const double* kcol, int k1, double* kv /*[QA]*/) {
+EXX_HD const double* k_line(const double* ks, int fullk, int kb, int tc, int p) {
+    const int sb = fullk ? kb : (kb <= C::TB - kb ? kb : C::TB - kb);
+    return ks + (static_cast<size_t>(sb) * tc + p) * (fullk ? C::TA : C::NSA);
+}
+template <class C>
+EXX_HD void b2_load_k(const double* kcol, int k1, double* kv /*[QA]*/, int fullk = 0) {
 #pragma unroll
     for (int k2 = 0; k2 < C::QA; ++k2) {
         const int ka = k1 + C::PA * k2;
-        kv[k2] = ld_ro(kcol + (ka <= C::TA - ka ? ka : C::TA - ka));
+        kv[k2] = ld_ro(kcol + (fullk || ka <= C::TA - ka ? ka : C::TA - ka));
     }
 }
 template <class C>
@@ -909,9 +918,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_b_kernel(const ArgsB g) {
                     const ColAIdx x = colp_index<C>(cg, lane + m * 32);
                     const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
                     const int kb = q + C::R1 * r;
-                    const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
                     double kv[C::QA];
-                    b2_load_k<C>(g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA, x.k, kv);
+                    b2_load_k<C>(k_line<C>(g.ks, g.fullk, kb, g.tc, pch * C::CHUNK + pin), x.k, kv, g.fullk);
                     b2_compute<C>(W + x.base, kv, TW2 + x.k, C::PA, x.k);
                 }
             __syncwarp();
@@ -1053,12 +1061,11 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
             const ColAIdx x = colp_index<C>(cg, w);
             const int r = x.col / C::CHUNK, pin = x.col % C::CHUNK;
             const int kb = q + C::R1 * r;
-            const int sb = kb <= C::TB - kb ? kb : C::TB - kb;
-            return g.ks + (static_cast<size_t>(sb) * g.tc + pch * C::CHUNK + pin) * C::NSA;
+            return k_line<C>(g.ks, g.fullk, kb, g.tc, pch * C::CHUNK + pin);
         };
         auto request_k = [&](int slice, int cg) {
             if (NP != 1 || (slice == k_slice && cg == k_cg)) return;
-            if (lane < C::ITEMS_P) b2_load_k<C>(kcol_of(slice, cg, lane), colp_index<C>(cg, lane).k, kv0);
+            if (lane < C::ITEMS_P) b2_load_k<C>(kcol_of(slice, cg, lane), colp_index<C>(cg, lane).k, kv0, g.fullk);
             k_slice = slice; k_cg = cg;
         };
         if (nk > 0 && wid < C::NGRP) request_k(id0 / g.count, wid);
@@ -1085,7 +1092,7 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
                         const int w = lane + m * 32;
                         const ColAIdx x = colp_index<C>(cg, w);
                         double kvm[C::QA];
-                        if (NP != 1) b2_load_k<C>(kcol_of(slice, cg, w), x.k, kvm);
+                        if (NP != 1) b2_load_k<C>(kcol_of(slice, cg, w), x.k, kvm, g.fullk);
                         const double* kv = NP == 1 ? kv0 : kvm;
                         if (SCRATCH) b2e_compute<C>(E + x.k * C::QRSE + w % C::NCW, kv, TW2 + x.k, C::PA, x.k);
                         else b2_compute<C>(W + x.base, kv, TW2 + x.k, C::PA, x.k);
@@ -1187,11 +1194,8 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     // The operand stage of transform t is refilled (for t + NSTG) by warp 0 once the reduce-adds of t have READ it.  Waiting
     // for that right after issuing them would idle warp 0 while the other warps already run C0 of t+1 and then wait for it
     // at the next barrier; instead the refill is deferred to after warp 0's own C0 of t+1, when the reads are long done.
-#ifdef EXX_C_REFILL_EAGER
-    constexpr bool DEFER = false;
-#else
-    constexpr bool DEFER = true;
-#endif
+    // (with a single stage the operand of t+1 would then arrive late: measured +3 % at 192^3, so only with two stages)
+    constexpr bool DEFER = NSTG >= 2;
     int refill_t = -1, refill_s = 0;
     for (int t = 0; t < g.count; ++t) {
         double2* S = S0 + (NBUF == 2 ? (t & 1) : 0) * C::SMEM_C;

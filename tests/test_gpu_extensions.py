@@ -4,6 +4,7 @@ tests/test_oracle_pins_ext.py.  Tolerances as in test_gpu_parity.py (north_star)
   exx_apply_to      K of the occupied set applied to another orbital set        (NEXT-1)
   periodic filter   host-supplied Fourier-space table (screened kernel)          (NEXT-2)
   slab / wire BC    FREE plan + one period of the mixed Green's function as data (NEXT-2)
+  general cells     non-orthorhombic periodic cell: K^ on the full FFT index grid   (NEXT-2)
   exx_apply_block   all pairs between two disjoint blocks + round-robin schedule (NEXT-3)
   exx_apply_pairs   sparse pair list for localised orbitals                      (NEXT-4)
 """
@@ -136,6 +137,30 @@ def test_slab_at_a_warp_specialised_size_matches_the_oracle():
     k_ref, ex_ref, _ = Oracle(spec.dims, spec.spacing, "free", table).apply(w["psi"].numpy(), occ)
     assert np.max(np.abs(kpsi.cpu().numpy() - k_ref)) <= K_RTOL * np.max(np.abs(k_ref))
     assert abs(ex - ex_ref) <= E_RTOL * abs(ex_ref)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ NEXT-2: general (non-orthorhombic) periodic cells
+@pytest.mark.parametrize("dims,n_orb,batch", [((16, 32, 64), 4, 0), ((96, 96, 96), 4, 2), ((48, 96, 32), 3, 0), ((192, 48, 96), 3, 2)])
+def test_general_cell_matches_oracle(dims, n_orb, batch):
+    """exx_plan_create_general: a triclinic cell -- K^ on the full FFT index grid, even only under inversion (DESIGN.md
+    A25) -- against the oracle with the same table (P16).  Orbitals: the seeded Gaussian sums sampled on the
+    index grid."""
+    from workloads import general_cell_khat
+    lattice = np.array([[0.5 * dims[0], 0.0, 0.0], [0.13 * dims[1], 0.45 * dims[1], 0.0], [-0.07 * dims[2], 0.1 * dims[2], 0.4 * dims[2]]])
+    khat, vol = general_cell_khat(dims, lattice)
+    w = make_workload(small_spec("C1", dims=dims, n_orb=n_orb, spacing=(0.45, 0.4, 0.5), number=1600 + sum(dims)))
+    occ = np.array([2.0, 1.2, 0.0, 0.7][:n_orb])
+    plan = exx.ExxPlan.general(dims, vol, khat, max_orbitals=n_orb)
+    if batch:
+        plan.set_batch(batch)
+    kpsi, ex = plan.apply(w["psi"].cuda(), occ)
+    k_ref, ex_ref, e_ref = Oracle.general(dims, vol, khat).apply(w["psi"].numpy(), occ)
+    assert np.max(np.abs(kpsi.cpu().numpy() - k_ref)) <= K_RTOL * np.max(np.abs(k_ref))
+    assert abs(ex - ex_ref) <= E_RTOL * abs(ex_ref)
+    e = plan.pair_energies(n_orb)
+    live = (occ[:, None] != 0) | (occ[None, :] != 0)
+    assert np.all((np.abs(e - e_ref) <= E_RTOL * np.max(np.abs(e_ref)))[live])
     plan.destroy()
 
 

@@ -96,6 +96,15 @@ def test_status_codes_without_compute():
     d = (C.c_int * 3)(36, 16, 16)                                                 # free BC: 2n = 72 mixed with 32
     g = np.ones(36 * 16 * 16)
     assert lib.exx_plan_create(C.byref(h), d, sp, 1, g.ctypes.data_as(C.POINTER(C.c_double)), 4, None) == 2
+    # exx_plan_create_general: argument checks come before any device work
+    d = (C.c_int * 3)(32, 32, 32)
+    k = np.ones(32 ** 3)
+    kp = k.ctypes.data_as(C.POINTER(C.c_double))
+    assert lib.exx_plan_create_general(C.byref(h), d, C.c_double(100.0), None, 4, None) == 1      # no table
+    assert lib.exx_plan_create_general(C.byref(h), d, C.c_double(-1.0), kp, 4, None) == 1         # volume <= 0
+    assert lib.exx_plan_create_general(C.byref(h), d, C.c_double(100.0), kp, 0, None) == 1        # max_orbitals < 1
+    d = (C.c_int * 3)(30, 32, 32)
+    assert lib.exx_plan_create_general(C.byref(h), d, C.c_double(100.0), kp, 4, None) == 2        # unsupported length
     assert lib.exx_plan_destroy(None) == 0
     assert lib.exx_plan_workspace_bytes(None) == 0
 

@@ -245,3 +245,63 @@ def test_p15_screened_image_table_is_even_and_decays():
     for ax in (0, 2):
         assert np.array_equal(g, np.take(g, (-np.arange(dims[ax])) % dims[ax], axis=ax))
     assert g[0, 0, 0] > g[1, 0, 0] > g[2, 0, 0] > 0 and g[0, 5, 0] < 1e-3 * g[0, 1, 0]
+
+
+# ------------------------------------------------------------------------------------------------ P16 general periodic cells
+TRICLINIC = np.array([[4.0, 0.0, 0.0], [1.1, 3.6, 0.0], [-0.7, 0.9, 4.4]])
+
+
+def test_p16_full_grid_filter_of_an_orthorhombic_cell_is_the_analytic_kernel():
+    from workloads import general_cell_khat
+    dims, spacing = (6, 4, 8), (0.5, 0.45, 0.4)
+    lattice = np.diag([n * h for n, h in zip(dims, spacing)])
+    khat, vol = general_cell_khat(dims, lattice)
+    rng = np.random.default_rng(1601)
+    rho = rng.standard_normal(dims)
+    want = Oracle(dims, spacing, "periodic").poisson(rho)
+    got = Oracle.general(dims, vol, khat).poisson(rho)
+    assert abs(vol - np.prod(lattice.diagonal())) <= 1e-12 * vol
+    assert np.max(np.abs(got - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+def test_p16_triclinic_plane_waves_read_their_own_table_entry():
+    """rho = cos / sin of the plane wave with FFT index m on the index grid -> V = K^[m] rho: the entry of exactly that
+    index (an asymmetric table would expose a transposed or mirrored lookup), for a cosine and -- since K^(-m) = K^(m) --
+    for a sine."""
+    from workloads import general_cell_khat
+    dims = (6, 8, 10)
+    khat, vol = general_cell_khat(dims, TRICLINIC)
+    o = Oracle.general(dims, vol, khat)
+    i, j, k = np.meshgrid(*[np.arange(n) for n in dims], indexing="ij")
+    for m in [(1, 2, 3), (5, 1, 0), (2, 7, 9), (0, 3, 8)]:
+        theta = 2 * np.pi * (m[0] * i / dims[0] + m[1] * j / dims[1] + m[2] * k / dims[2])
+        for f in (np.cos, np.sin):
+            v = o.poisson(f(theta))
+            assert np.max(np.abs(v - khat[m] * f(theta))) <= 1e-13 * khat[m]
+    # the table is not even in each index separately (that is what makes the cell "general") but inversion-symmetric
+    assert abs(khat[1, 2, 3] - khat[5, 2, 3]) > 1e-3 * khat[1, 2, 3]
+    assert khat[1, 2, 3] == khat[5, 6, 7]
+
+
+def test_p16_triclinic_fft_path_is_the_brute_force_convolution():
+    from workloads import general_cell_khat
+    dims = (4, 6, 4)
+    khat, vol = general_cell_khat(dims, TRICLINIC)
+    o = Oracle.general(dims, vol, khat)
+    rng = np.random.default_rng(1602)
+    rho = rng.standard_normal(dims)
+    v, vd = o.poisson(rho), o.poisson_direct(rho)
+    assert np.max(np.abs(v - vd)) <= 1e-12 * np.max(np.abs(v))
+
+
+def test_p16_triclinic_coulomb_entry_is_four_pi_over_g_squared():
+    """One entry of the seeded table against the textbook reciprocal-lattice construction b1 = 2 pi (a2 x a3) / V, ..."""
+    from workloads import general_cell_khat
+    dims = (6, 8, 10)
+    khat, vol = general_cell_khat(dims, TRICLINIC)
+    a1, a2, a3 = TRICLINIC
+    v = float(np.dot(a1, np.cross(a2, a3)))
+    b1, b2, b3 = (2 * np.pi * np.cross(a2, a3) / v, 2 * np.pi * np.cross(a3, a1) / v, 2 * np.pi * np.cross(a1, a2) / v)
+    g = 1 * b1 + (-2) * b2 + 3 * b3                      # index (1, 6, 3) <-> frequencies (1, -2, 3)
+    assert abs(vol - abs(v)) <= 1e-12 * abs(v)
+    assert abs(khat[1, 6, 3] - 4 * np.pi / np.dot(g, g)) <= 1e-13 * khat[1, 6, 3]

@@ -11,6 +11,7 @@ from .generator import (  # noqa: F401
     WorkloadSpec,
     cell_average_inverse_r,
     free_kernel_table,
+    general_cell_khat,
     make_orbitals,
     make_workload,
     mixed_bc_kernel_table,

@@ -249,6 +249,26 @@ def mixed_bc_kernel_table(dims, spacing, periodic, mu: float, images: int = 2) -
     return np.ascontiguousarray(g)
 
 
+def general_cell_khat(dims, lattice) -> tuple:
+    """Fourier-space Coulomb kernel of a periodic cell of any shape, for exx_plan_create_general: lattice = rows a1, a2, a3
+    (bohr).  Returns (K^ on the full FFT index grid [n1][n2][n3], cell volume):  K^(m) = 4 pi / |m1 b1 + m2 b2 + m3 b3|^2
+    with the reciprocal vectors b_a (a_a . b_b = 2 pi delta_ab) and signed frequencies m_a in (-n_a/2, n_a/2], K^(0) = 0.
+    An index n_a/2 is its own negative, so the table is symmetrised, K^(m) <- (K^(m) + K^(-m mod n)) / 2, which makes
+    K^(-m) = K^(m) hold exactly (real potentials).  Input data only: none of the method's arithmetic."""
+    n = [int(d) for d in dims]
+    a = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
+    vol = abs(float(np.linalg.det(a)))
+    b = 2.0 * np.pi * np.linalg.inv(a).T                    # rows b1, b2, b3
+    m = [np.where(np.arange(k) <= k // 2, np.arange(k), np.arange(k) - k).astype(np.float64) for k in n]
+    g = (m[0][:, None, None, None] * b[0] + m[1][None, :, None, None] * b[1] + m[2][None, None, :, None] * b[2])
+    g2 = np.sum(g * g, axis=-1)
+    khat = np.where(g2 > 0, 4.0 * np.pi / np.where(g2 > 0, g2, 1.0), 0.0)
+    neg = khat
+    for ax in range(3):
+        neg = np.take(neg, (-np.arange(n[ax])) % n[ax], axis=ax)
+    return np.ascontiguousarray(0.5 * (khat + neg)), vol
+
+
 def make_workload(spec_or_name, device="cpu") -> dict:
     """Orbitals, occupations and (free BC) the Green's-function table for a config name or a WorkloadSpec."""
     spec = CONFIGS[spec_or_name] if isinstance(spec_or_name, str) else spec_or_name
