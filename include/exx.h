@@ -153,6 +153,29 @@ exx_status exx_apply_to(exx_plan *plan, int n_occ, const double *psi_dev, const 
                         const double *phi_dev, double *kphi_dev);
 
 /*
+ * exx_apply_to_cross -- exx_apply_to with a partner set: the potential of the co-density (phi_t, psi_j) is multiplied by
+ * chi_j instead of psi_j,
+ *      K phi_t (r) = - sum_j f_j  V[phi_t psi_j](r)  chi_j(r),
+ * the building block that the real and imaginary parts of complex orbitals need (below).  chi_dev DEVICE
+ * [n_occ][n1][n2][n3]; everything else as exx_apply_to.
+ *
+ * exx_apply_complex -- the hot path for COMPLEX orbitals psi = u + i v (Eq. 8 keeps the conjugate; the
+ * paper's own runs are real, Gamma point, :159):  rho_ij = conj(psi_j) psi_i,  K psi_i = - sum_j f_j V_ij psi_j,
+ * E_x = -1/2 sum f_i f_j <rho_ij|V_ij>  (reading A26).  Computed with the real kernels from the 2 n_orb real
+ * orbitals X = (u_1..u_N, v_1..v_N):  A = K[X] X (exx_apply),  B = the cross term of X with the partner set (-v, u)
+ * (exx_apply_to_cross),  K psi = (A[u] + B[v]) + i (A[v] - B[u]),  E_x = 1/2 dV sum_i f_i Re<psi_i|K psi_i>.
+ *   psi_dev   DEVICE, PLANAR [2][n_orb][n1][n2][n3]: all real parts, then all imaginary parts; read-only.
+ *   kpsi_dev  DEVICE, same layout, OVERWRITTEN.
+ *   work_dev  DEVICE, caller-owned scratch of 6 * n_orb * n1*n2*n3 doubles, 16-byte aligned (no allocation happens here).
+ *   occ_host  HOST [n_orb];  ex_host HOST.   Needs 2 * n_orb <= max_orbitals.  Costs 6 n_orb^2 real pair solves (a native
+ *   complex prologue / epilogue would need 2 n_orb^2: correctness first).  Synchronises.
+ */
+exx_status exx_apply_to_cross(exx_plan *plan, int n_occ, const double *psi_dev, const double *chi_dev, const double *occ_host,
+                              int n_tgt, const double *phi_dev, double *kphi_dev);
+exx_status exx_apply_complex(exx_plan *plan, int n_orb, const double *psi_dev, const double *occ_host, double *kpsi_dev,
+                             double *work_dev, double *ex_host);
+
+/*
  * exx_apply_block -- all pairs BETWEEN two disjoint orbital blocks, the unit of work of the paper's round-robin
  * distribution (Fig. 1: each process "calculates the co-densities between its own orbitals and the
  * received ones"; the potential serves both orbitals of a pair):  for every j in the resident block, i in the streamed one

@@ -199,6 +199,37 @@ class Oracle:
             raise RuntimeError(f"exx_oracle_apply_to failed ({rc})")
         return kphi.reshape((n_tgt,) + self.dims)
 
+    def apply_to_cross(self, psi, chi, occ, phi):
+        """K phi_t = - sum_j f_j V[phi_t psi_j] chi_j: the potential of the co-density (phi_t, psi_j) multiplied by a partner
+        orbital chi_j (chi = psi gives apply_to).  Plain numpy loop over the pairs on top of the pinned Poisson solve."""
+        psi, chi, phi = (_f64(x).reshape((-1,) + self.dims) for x in (psi, chi, phi))
+        occ = _f64(occ)
+        out = np.zeros_like(phi)
+        for t in range(phi.shape[0]):
+            for j in range(psi.shape[0]):
+                if occ[j] != 0.0:
+                    out[t] -= occ[j] * self.poisson(phi[t] * psi[j]) * chi[j]
+        return out
+
+    def apply_complex(self, psi, occ):
+        """Complex orbitals (Eq. 8 with its conjugate; reading A26), the definition over all ordered
+        pairs:  rho = conj(psi_j) psi_i,  V = Poisson(Re rho) + i Poisson(Im rho)  (the Green's function is real),
+        K psi_i -= f_j V psi_j,  E_x -= 1/2 f_i f_j dV sum_r conj(rho) V.  Returns (K psi complex, E_x)."""
+        psi = np.ascontiguousarray(np.asarray(psi, dtype=np.complex128)).reshape((-1,) + self.dims)
+        occ = _f64(occ)
+        n = psi.shape[0]
+        kpsi = np.zeros_like(psi)
+        ex = 0.0
+        for i in range(n):
+            for j in range(n):
+                if occ[i] == 0.0 and occ[j] == 0.0:
+                    continue
+                rho = np.conj(psi[j]) * psi[i]
+                v = self.poisson(rho.real) + 1j * self.poisson(rho.imag)
+                kpsi[i] -= occ[j] * v * psi[j]
+                ex -= 0.5 * occ[i] * occ[j] * self.dV * float(np.sum(np.conj(rho) * v).real)
+        return kpsi, ex
+
     def apply_block(self, psi_a, occ_a, psi_b, occ_b):
         """All pairs between two disjoint blocks: returns (ka, kb, ex, e_block[n_a, n_b])."""
         psi_a = _f64(psi_a)

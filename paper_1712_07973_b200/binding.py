@@ -23,7 +23,7 @@ _STATUS = ["EXX_OK", "EXX_ERR_INVALID_ARG", "EXX_ERR_UNSUPPORTED_SIZE", "EXX_ERR
 EXX_BLOCK_ACCUMULATE_RESIDENT, EXX_BLOCK_ACCUMULATE_STREAMED = 1, 2
 
 EXPORTS = [
-    "exx_plan_create", "exx_plan_create_general", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_apply_pairs", "exx_apply_to", "exx_apply_block",
+    "exx_plan_create", "exx_plan_create_general", "exx_apply", "exx_apply_async", "exx_apply_host", "exx_apply_pairs", "exx_apply_to", "exx_apply_to_cross", "exx_apply_complex", "exx_apply_block",
     "exx_get_pair_energies", "exx_get_block_energies", "exx_plan_release_staging",
     "exx_schedule_pairs", "exx_schedule_list", "exx_schedule_list_masked", "exx_schedule_list_block", "exx_round_robin_step",
     "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_device", "exx_plan_kernel_name",
@@ -72,6 +72,10 @@ def load_library():
     lib.exx_apply_pairs.restype = C.c_int
     lib.exx_apply_to.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_int, C.c_void_p, C.c_void_p]
     lib.exx_apply_to.restype = C.c_int
+    lib.exx_apply_to_cross.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, _dp, C.c_int, C.c_void_p, C.c_void_p]
+    lib.exx_apply_to_cross.restype = C.c_int
+    lib.exx_apply_complex.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]
+    lib.exx_apply_complex.restype = C.c_int
     lib.exx_apply_block.argtypes = [C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_int, C.c_void_p, _dp, C.c_void_p, C.c_int,
                                     C.c_void_p]
     lib.exx_apply_block.restype = C.c_int
@@ -380,6 +384,39 @@ class ExxPlan:
                                          int(phi.shape[0]), C.c_void_p(phi.data_ptr()), C.c_void_p(kphi.data_ptr()))
         self._check(st)
         return kphi
+
+    def apply_to_cross(self, psi, chi, occ, phi, kphi=None):
+        """exx_apply_to_cross: kphi_t = - sum_j f_j V[phi_t psi_j] chi_j."""
+        import torch
+        self._check_dev(psi, "psi")
+        self._check_dev(chi, "chi", int(psi.shape[0]))
+        self._check_dev(phi, "phi")
+        kphi = torch.empty_like(phi) if kphi is None else self._check_dev(kphi, "kphi", int(phi.shape[0]))
+        occ = self._occ(occ, int(psi.shape[0]))
+        st = load_library().exx_apply_to_cross(self._h, int(psi.shape[0]), C.c_void_p(psi.data_ptr()), C.c_void_p(chi.data_ptr()),
+                                               occ.ctypes.data_as(_dp), int(phi.shape[0]), C.c_void_p(phi.data_ptr()),
+                                               C.c_void_p(kphi.data_ptr()))
+        self._check(st)
+        return kphi
+
+    def apply_complex(self, psi_planar, occ, kpsi_planar=None, work=None):
+        """exx_apply_complex: psi_planar = CUDA fp64 [2, N, n1, n2, n3] (real parts, imaginary parts); returns (kpsi_planar, E_x)."""
+        import torch
+        if not (isinstance(psi_planar, torch.Tensor) and psi_planar.dim() == 5 and psi_planar.shape[0] == 2):
+            raise ValueError("psi_planar must have shape (2, N, n1, n2, n3)")
+        n = int(psi_planar.shape[1])
+        x = self._check_dev(psi_planar.view(2 * n, *self.dims), "psi_planar")
+        kpsi_planar = torch.empty_like(psi_planar) if kpsi_planar is None else kpsi_planar
+        k = self._check_dev(kpsi_planar.view(2 * n, *self.dims), "kpsi_planar", 2 * n)
+        work = torch.empty(6 * n * x[0].numel(), dtype=torch.float64, device=psi_planar.device) if work is None else work
+        if not (work.is_cuda and work.dtype == torch.float64 and work.is_contiguous() and work.numel() >= 6 * n * x[0].numel()):
+            raise ValueError("work must be a contiguous CUDA float64 tensor of at least 6 N n1 n2 n3 elements")
+        occ = self._occ(occ, n)
+        ex = C.c_double()
+        st = load_library().exx_apply_complex(self._h, n, C.c_void_p(x.data_ptr()), occ.ctypes.data_as(_dp), C.c_void_p(k.data_ptr()),
+                                              C.c_void_p(work.data_ptr()), C.byref(ex))
+        self._check(st)
+        return kpsi_planar, ex.value
 
     def apply_block(self, psi_res, occ_res, kpsi_res, psi_str, occ_str, kpsi_str, flags=0):
         """exx_apply_block: all pairs between two disjoint blocks; returns the block's contribution to E_x."""

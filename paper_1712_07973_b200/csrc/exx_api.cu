@@ -173,6 +173,50 @@ __global__ void exchange_energy_kernel(const double* e_mat, const double* occ_r,
     if (threadIdx.x == 0) *ex = scale * sh[0];
 }
 
+// Complex orbitals psi = u + i v by real building blocks (exx_apply_complex).  X = (u_1..u_N, v_1..v_N) is the caller's
+// planar array; jx = (-v_1..-v_N, u_1..u_N) is the partner set of the cross term.
+__global__ void complex_partner_kernel(const double* x, double* jx, long long nm) {      // nm = N * M
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < nm;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        jx[k] = -x[nm + k];
+        jx[nm + k] = x[k];
+    }
+}
+// K psi = (A[u] + B[v]) + i (A[v] - B[u]) written over out = [2][N][M]; per-block partial sums of
+// sum_i f_i Re <psi_i | K psi_i> = sum_i f_i sum_r (u_i Kre_i + v_i Kim_i) in a fixed order (deterministic).
+__global__ void complex_combine_kernel(const double* x, const double* a, const double* b, const double* occ, double* out,
+                                       long long m_points, int n_orb, double* partial) {
+    __shared__ double sh[256];
+    const long long nm = m_points * n_orb;
+    double s = 0.0;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < nm;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const double kre = a[k] + b[nm + k], kim = a[nm + k] - b[k];
+        out[k] = kre;
+        out[nm + k] = kim;
+        s += occ[k / m_points] * (x[k] * kre + x[nm + k] * kim);
+    }
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void complex_energy_kernel(const double* partial, int n, double scale, double* ex) {
+    __shared__ double sh[256];
+    double s = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) s += partial[k];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *ex = scale * sh[0];
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------ plan
@@ -218,6 +262,7 @@ struct exx_plan {
     size_t events_used;
     Schedule sched;         // reserved for the largest apply at creation: exx_apply* allocate nothing
     std::vector<char> copied;   // exx_apply_host: rows of K psi already on their way to the host
+    std::vector<double> occ2;   // exx_apply_complex: occupations (f, f) of the 2N real orbitals (reserved at creation)
     size_t ws_bytes;        // batch workspace (W1 + energy partials)
     size_t fixed_bytes;     // tables, descriptors, pair-energy matrix
     std::string err;
@@ -448,6 +493,7 @@ struct Job {
     int n_res, n_str;               // square: both = n_orb
     const double* psi_res;
     const double* psi_str;
+    const double* psi_str_epi;      // nullptr, or the set pass C multiplies the potentials with instead of psi_str (exx_apply_to_cross)
     double* kpsi_res;               // nullptr: the resident side receives nothing
     double* kpsi_str;               // nullptr: the streamed side receives nothing
     const double* occ_res;          // host; nullptr: all zero (exx_apply_to)
@@ -513,7 +559,13 @@ exx_status run_job_unguarded(exx_plan* p, const Job& job) {
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_b(p->geo, ab, b.count, s, nullptr));
         EXX_CUDA(p, mark());
-        EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
+        if (job.psi_str_epi) {                             // Kernel 3 multiplies V[phi psi_i] with chi_i instead of psi_i
+            ArgsAC acc = ac;
+            acc.psi = job.psi_str_epi;
+            EXX_CUDA(p, launch_pass_c(p->geo, acc, s, nullptr));
+        } else {
+            EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
+        }
         EXX_CUDA(p, mark());
         p->launches += 3;
         if (job.energy) {
@@ -796,6 +848,7 @@ static exx_status create_impl(exx_plan** plan, const int dims[3], const double s
     try {
         reserve_schedule(p->sched, static_cast<size_t>(max_orbitals), static_cast<size_t>(max_orbitals));
         p->copied.assign(static_cast<size_t>(max_orbitals), 0);
+        p->occ2.reserve(static_cast<size_t>(max_orbitals));
     } catch (const std::bad_alloc&) {
         return bail(fail(p, EXX_ERR_ALLOC, "out of host memory (schedule storage)"));
     }
@@ -1009,23 +1062,25 @@ exx_status exx_apply_pairs(exx_plan* p, int n_orb, const double* psi_dev, const 
     return finish_sync(p, ex_host);
 }
 
-exx_status exx_apply_to(exx_plan* p, int n_occ, const double* psi_dev, const double* occ_host, int n_tgt, const double* phi_dev,
-                        double* kphi_dev) {
-    if (!p) return EXX_ERR_INVALID_ARG;
-    if (!psi_dev || !occ_host || !phi_dev || !kphi_dev) return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
-    EXX_ENTER(p);
+static exx_status apply_to_impl(exx_plan* p, int n_occ, const double* psi_dev, const double* chi_dev, const double* occ_host, int n_tgt,
+                                const double* phi_dev, double* kphi_dev, bool sync) {
     exx_status st = check_set(p, n_occ, psi_dev, nullptr, "exx_apply_to (occupied set)");
     if (st != EXX_OK) return st;
+    if (chi_dev) {
+        st = check_set(p, n_occ, chi_dev, nullptr, "exx_apply_to_cross (partner set)");
+        if (st != EXX_OK) return st;
+    }
     st = check_set(p, n_tgt, phi_dev, kphi_dev, "exx_apply_to (target set)");
     if (st != EXX_OK) return st;
     if (is_device_pointer(occ_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host must be a host pointer");
     const size_t e_occ = static_cast<size_t>(n_occ) * p->M, e_tgt = static_cast<size_t>(n_tgt) * p->M;
-    if (ranges_overlap(kphi_dev, e_tgt, psi_dev, e_occ) || ranges_overlap(kphi_dev, e_tgt, phi_dev, e_tgt))
-        return fail(p, EXX_ERR_INVALID_ARG, "kphi must not overlap psi or phi");
+    if (ranges_overlap(kphi_dev, e_tgt, psi_dev, e_occ) || ranges_overlap(kphi_dev, e_tgt, phi_dev, e_tgt) ||
+        (chi_dev && ranges_overlap(kphi_dev, e_tgt, chi_dev, e_occ)))
+        return fail(p, EXX_ERR_INVALID_ARG, "kphi must not overlap psi, chi or phi");
     Job job{};
     job.square = false;
     job.n_res = n_tgt; job.n_str = n_occ;
-    job.psi_res = phi_dev; job.psi_str = psi_dev;
+    job.psi_res = phi_dev; job.psi_str = psi_dev; job.psi_str_epi = chi_dev;
     job.kpsi_res = kphi_dev; job.kpsi_str = nullptr;
     job.occ_res = nullptr; job.occ_str = occ_host;
     job.zero_res = true;
@@ -1033,8 +1088,69 @@ exx_status exx_apply_to(exx_plan* p, int n_occ, const double* psi_dev, const dou
     job.energy = false;
     st = run_job(p, job);
     if (st != EXX_OK) return st;
-    EXX_CUDA(p, cudaStreamSynchronize(p->stream));
+    if (sync) EXX_CUDA(p, cudaStreamSynchronize(p->stream));
     return EXX_OK;
+}
+
+exx_status exx_apply_to(exx_plan* p, int n_occ, const double* psi_dev, const double* occ_host, int n_tgt, const double* phi_dev,
+                        double* kphi_dev) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    if (!psi_dev || !occ_host || !phi_dev || !kphi_dev) return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
+    EXX_ENTER(p);
+    return apply_to_impl(p, n_occ, psi_dev, nullptr, occ_host, n_tgt, phi_dev, kphi_dev, true);
+}
+
+exx_status exx_apply_to_cross(exx_plan* p, int n_occ, const double* psi_dev, const double* chi_dev, const double* occ_host, int n_tgt,
+                              const double* phi_dev, double* kphi_dev) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    if (!psi_dev || !chi_dev || !occ_host || !phi_dev || !kphi_dev) return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
+    EXX_ENTER(p);
+    return apply_to_impl(p, n_occ, psi_dev, chi_dev, occ_host, n_tgt, phi_dev, kphi_dev, true);
+}
+
+exx_status exx_apply_complex(exx_plan* p, int n_orb, const double* psi_dev, const double* occ_host, double* kpsi_dev, double* work_dev,
+                             double* ex_host) {
+    if (!p) return EXX_ERR_INVALID_ARG;
+    if (!psi_dev || !occ_host || !kpsi_dev || !work_dev || !ex_host) return fail(p, EXX_ERR_INVALID_ARG, "NULL argument");
+    if (n_orb < 1 || 2 * static_cast<long long>(n_orb) > p->max_orb)
+        return fail(p, EXX_ERR_INVALID_ARG, "exx_apply_complex needs 2 * n_orb <= max_orbitals");
+    EXX_ENTER(p);
+    if (!is_device_pointer(work_dev) || !aligned16(work_dev)) return fail(p, EXX_ERR_BAD_POINTER, "work_dev must be 16-byte aligned device memory");
+    if (is_device_pointer(occ_host) || is_device_pointer(ex_host)) return fail(p, EXX_ERR_BAD_POINTER, "occ_host and ex_host must be host pointers");
+    const int n2 = 2 * n_orb;
+    const size_t nm = static_cast<size_t>(n_orb) * p->M, set = 2 * nm;
+    exx_status st = check_set(p, n2, psi_dev, kpsi_dev, "exx_apply_complex");
+    if (st != EXX_OK) return st;
+    if (ranges_overlap(work_dev, 3 * set, psi_dev, set) || ranges_overlap(work_dev, 3 * set, kpsi_dev, set) ||
+        ranges_overlap(psi_dev, set, kpsi_dev, set))
+        return fail(p, EXX_ERR_INVALID_ARG, "psi, kpsi and work must not overlap");
+    double* jx = work_dev;                                 // partner set (-v, u)
+    double* ka = work_dev + set;                           // A = K[X] X      (square apply of the 2N real orbitals)
+    double* kb = work_dev + 2 * set;                       // B = T(X, JX) X  (cross term)
+    // the 2N real orbitals carry the occupations (f, f); the pinned occupation staging doubles as the host copy
+    try {
+        p->occ2.assign(static_cast<size_t>(n2), 0.0);
+    } catch (const std::bad_alloc&) {
+        return fail(p, EXX_ERR_ALLOC, "out of host memory");
+    }
+    for (int k = 0; k < n_orb; ++k) p->occ2[k] = p->occ2[n_orb + k] = occ_host[k];
+    cudaStream_t s = p->stream;
+    complex_partner_kernel<<<2048, 256, 0, s>>>(psi_dev, jx, static_cast<long long>(nm));
+    EXX_CUDA(p, cudaGetLastError());
+    ++p->launches;
+    st = square_device_apply(p, n2, psi_dev, p->occ2.data(), nullptr, ka);
+    if (st != EXX_OK) return st;
+    st = apply_to_impl(p, n2, psi_dev, jx, p->occ2.data(), n2, psi_dev, kb, false);
+    if (st != EXX_OK) return st;
+    // occupations of the orbitals on the device: run_job left (f, f) in occ_dev + max_orb (the streamed set's columns)
+    const long long ep_cap = static_cast<long long>(p->max_batch) * p->info_c.tiles * 2;   // doubles in the partial-sum buffer
+    const int nblk = static_cast<int>(ep_cap < 1024 ? (ep_cap < 1 ? 1 : ep_cap) : 1024);
+    complex_combine_kernel<<<nblk, 256, 0, s>>>(psi_dev, ka, kb, p->occ_dev + p->max_orb, kpsi_dev, p->M, n_orb, p->epart);
+    complex_energy_kernel<<<1, 256, 0, s>>>(p->epart, nblk, 0.5 * p->dV, p->ex_dev);
+    EXX_CUDA(p, cudaGetLastError());
+    p->launches += 2;
+    p->last_rows = p->last_cols = 0;
+    return finish_sync(p, ex_host);
 }
 
 exx_status exx_apply_block(exx_plan* p, int n_res, const double* psi_res_dev, const double* occ_res_host, double* kpsi_res_dev, int n_str,

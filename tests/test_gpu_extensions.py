@@ -2,6 +2,7 @@
 tests/test_oracle_pins_ext.py.  Tolerances as in test_gpu_parity.py (north_star): 1e-10 max|K psi|, 1e-11 on energies.
 
   exx_apply_to      K of the occupied set applied to another orbital set        (NEXT-1)
+  exx_apply_complex complex orbitals through the real kernels (+ exx_apply_to_cross)  (NEXT-1; Eq. 8)
   periodic filter   host-supplied Fourier-space table (screened kernel)          (NEXT-2)
   slab / wire BC    FREE plan + one period of the mixed Green's function as data (NEXT-2)
   general cells     non-orthorhombic periodic cell: K^ on the full FFT index grid   (NEXT-2)
@@ -54,6 +55,36 @@ def test_apply_to_matches_oracle(base, dims, n_occ, n_tgt, batch):
     # a second "spin channel" is a second call with other occupied orbitals on the same plan: results are independent
     kphi2 = plan.apply_to(psi, occ, phi)
     assert torch.equal(kphi, kphi2)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ NEXT-1: complex orbitals
+@pytest.mark.parametrize("base,dims,n_orb,batch", [("C1", (16, 16, 16), 3, 0), ("C2", (8, 16, 8), 3, 2), ("C1", (96, 96, 96), 3, 3),
+                                                   ("C2", (48, 48, 48), 2, 0)])
+def test_apply_complex_matches_oracle(base, dims, n_orb, batch):
+    """exx_apply_complex (planar real / imaginary parts) against the oracle's complex definition (P17), and its building
+    block exx_apply_to_cross against the oracle's cross apply."""
+    w = make_workload(small_spec(base, dims=dims, n_orb=2 * n_orb, spacing=(0.45, 0.4, 0.5), number=1700 + sum(dims)))
+    spec = w["spec"]
+    plan = exx.ExxPlan(spec.dims, spec.spacing, spec.bc, w["kernel"], max_orbitals=2 * n_orb)
+    if batch:
+        plan.set_batch(batch)
+    o = Oracle(spec.dims, spec.spacing, spec.bc, w["kernel"])
+    planar = w["psi"].reshape(2, n_orb, *dims)                              # seeded real / imaginary parts
+    psi_c = planar[0].numpy() + 1j * planar[1].numpy()
+    occ = np.array([2.0, 0.9, 0.0][:n_orb])
+    k_ref, ex_ref = o.apply_complex(psi_c, occ)
+    kpl, ex = plan.apply_complex(planar.cuda(), occ)
+    k_gpu = kpl[0].cpu().numpy() + 1j * kpl[1].cpu().numpy()
+    assert np.max(np.abs(k_gpu - k_ref)) <= K_RTOL * np.max(np.abs(k_ref))
+    assert abs(ex - ex_ref) <= E_RTOL * abs(ex_ref)
+    # the building block on its own
+    x = w["psi"].cuda()
+    chi = torch.flip(x, dims=[0]).contiguous()
+    occ2 = np.concatenate([occ, occ])
+    kx = plan.apply_to_cross(x, chi, occ2, x[:2].contiguous())
+    ref = o.apply_to_cross(w["psi"].numpy(), chi.cpu().numpy(), occ2, w["psi"][:2].numpy())
+    assert np.max(np.abs(kx.cpu().numpy() - ref)) <= K_RTOL * np.max(np.abs(ref))
     plan.destroy()
 
 

@@ -305,3 +305,75 @@ def test_p16_triclinic_coulomb_entry_is_four_pi_over_g_squared():
     g = 1 * b1 + (-2) * b2 + 3 * b3                      # index (1, 6, 3) <-> frequencies (1, -2, 3)
     assert abs(vol - abs(v)) <= 1e-12 * abs(v)
     assert abs(khat[1, 6, 3] - 4 * np.pi / np.dot(g, g)) <= 1e-13 * khat[1, 6, 3]
+
+
+# ------------------------------------------------------------------------------------------------ P17 complex orbitals
+def _complex_set(seed, dims, n):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((n,) + dims) + 1j * rng.standard_normal((n,) + dims)
+
+
+def test_p17_real_orbitals_reduce_to_the_real_apply():
+    for bc, dims in (("periodic", (6, 4, 8)), ("free", (4, 6, 4))):
+        w = make_workload(small_spec("C1" if bc == "periodic" else "C2", dims=dims, n_orb=3, spacing=(0.5, 0.45, 0.4), number=1701))
+        o = Oracle(dims, w["spec"].spacing, bc, w["kernel"])
+        occ = np.array([2.0, 0.0, 1.1])
+        k_ref, ex_ref, _ = o.apply(w["psi"].numpy(), occ)
+        k, ex = o.apply_complex(w["psi"].numpy().astype(np.complex128), occ)
+        assert np.max(np.abs(k.imag)) == 0.0
+        assert np.max(np.abs(k.real - k_ref)) <= 1e-13 * np.max(np.abs(k_ref))
+        assert abs(ex - ex_ref) <= 1e-13 * abs(ex_ref)
+
+
+def test_p17_plane_wave_exchange_closed_form():
+    """psi_n = Vol^-1/2 exp(i k_n.r): rho_ij = exp(i (k_i - k_j).r) / Vol, V_ij = 4 pi / |k_i - k_j|^2 rho_ij (0 for i = j), so
+    K psi_i = - [sum_{j != i} f_j 4 pi / (|k_i - k_j|^2 Vol)] psi_i  and  E_x = -1/2 sum_{i != j} f_i f_j 4 pi / (|k_i - k_j|^2 Vol):
+    the textbook exchange of plane waves.  A missing conjugate turns k_i - k_j into k_i + k_j."""
+    dims, spacing = (8, 6, 10), (0.5, 0.45, 0.4)
+    L = np.array([n * h for n, h in zip(dims, spacing)])
+    vol = float(np.prod(L))
+    ms = [(1, 0, 2), (2, 1, 0), (-1, 2, 1)]
+    ks = [2 * np.pi * np.array(m) / L for m in ms]
+    X, Y, Z = _grid(dims, spacing)
+    psi = np.stack([np.exp(1j * (k[0] * X + k[1] * Y + k[2] * Z)) / np.sqrt(vol) for k in ks])
+    occ = np.array([2.0, 1.0, 0.5])
+    k_got, ex_got = Oracle(dims, spacing, "periodic").apply_complex(psi, occ)
+    ex_want = 0.0
+    for i in range(3):
+        lam = sum(occ[j] * 4 * np.pi / (np.dot(ks[i] - ks[j], ks[i] - ks[j]) * vol) for j in range(3) if j != i)
+        assert np.max(np.abs(k_got[i] + lam * psi[i])) <= 1e-13 * lam * np.max(np.abs(psi[i]))
+        ex_want -= 0.5 * occ[i] * lam
+    assert abs(ex_got - ex_want) <= 1e-13 * abs(ex_want)
+
+
+def test_p17_phase_covariance_hermiticity_and_energy_identity():
+    dims, spacing = (4, 6, 4), (0.5, 0.45, 0.4)
+    w = make_workload(small_spec("C2", dims=dims, n_orb=3, spacing=spacing, number=1702))
+    o = Oracle(dims, spacing, "free", w["kernel"])
+    psi = _complex_set(1703, dims, 3)
+    occ = np.array([2.0, 0.8, 1.4])
+    k, ex = o.apply_complex(psi, occ)
+    # every orbital may carry its own phase: K (e^{i t_i} psi_i) = e^{i t_i} K psi_i, E_x unchanged
+    ph = np.exp(1j * np.array([0.3, -1.1, 2.0]))[:, None, None, None]
+    k2, ex2 = o.apply_complex(ph * psi, occ)
+    assert np.max(np.abs(k2 - ph * k)) <= 1e-12 * np.max(np.abs(k))
+    assert abs(ex2 - ex) <= 1e-12 * abs(ex)
+    # <psi_a|K psi_b> is Hermitian;  E_x = 1/2 dV sum f_i Re<psi_i|K psi_i> <= 0
+    m = np.einsum("axyz,bxyz->ab", np.conj(psi), k)
+    assert np.max(np.abs(m - m.conj().T)) <= 1e-12 * np.max(np.abs(m))
+    assert ex < 0 and abs(ex - 0.5 * o.dV * float(np.sum(occ * np.diag(m).real))) <= 1e-12 * abs(ex)
+
+
+def test_p17_cross_apply_reduces_to_apply_to_and_is_linear_in_the_partner():
+    dims, spacing = (4, 6, 4), (0.5, 0.45, 0.4)
+    w = make_workload(small_spec("C2", dims=dims, n_orb=5, spacing=spacing, number=1704))
+    o = Oracle(dims, spacing, "free", w["kernel"])
+    allp = w["psi"].numpy()
+    psi, phi = allp[:3], allp[3:]
+    occ = np.array([2.0, 0.0, 1.3])
+    assert np.max(np.abs(o.apply_to_cross(psi, psi, occ, phi) - o.apply_to(psi, occ, phi))) <= 1e-13 * np.max(np.abs(phi))
+    rng = np.random.default_rng(1705)
+    c1, c2 = rng.standard_normal(psi.shape), rng.standard_normal(psi.shape)
+    lhs = o.apply_to_cross(psi, 2.0 * c1 - 0.5 * c2, occ, phi)
+    rhs = 2.0 * o.apply_to_cross(psi, c1, occ, phi) - 0.5 * o.apply_to_cross(psi, c2, occ, phi)
+    assert np.max(np.abs(lhs - rhs)) <= 1e-12 * np.max(np.abs(rhs))
