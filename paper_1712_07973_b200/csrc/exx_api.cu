@@ -12,6 +12,7 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>               // CUtensorMap + the prototype of cuTensorMapEncodeTiled (resolved at run time, libcuda is not linked)
 #include <nvtx3/nvToolsExt.h>   // header-only; the ranges cost nothing unless a tool (nsys, ncu --nvtx) attaches
 
 #include "../../include/exx.h"
@@ -232,6 +233,7 @@ struct exx_plan {
     cudaStream_t stream;
     double2* tw[3];
     double2* twb;           // [b2*R1 + q] = W_TB^{b2 q}
+    double2* twc_rot;       // [n2*NCLS + cls] = W_TC^{n2 (k1 + PC r)}: the rotated c-axis twiddles of pass C's TMA-gather variant
     double* ks;             // [TB/2+1][TC][TA/2+1], c index in scrambled order (see permute_kernel_axes)
     double2* w1;
     size_t w1_elems_per_xform;
@@ -251,6 +253,7 @@ struct exx_plan {
     double* kpsi_stage;
     size_t stage_elems;
     KernelInfo info_a, info_b, info_c;
+    alignas(64) unsigned char w1_map[128];   // CUtensorMap of W1 for pass C's TMA tile gather (info_c.needs_w1_map)
     long long launches;
     int device;             // ordinal of the device the plan was created on; every entry point switches to it
     int last_rows, last_cols;   // shape of the energy matrix the most recent apply left in e_mat (0: none)
@@ -356,6 +359,34 @@ exx_status grow_event_pool(exx_plan* p) {
     return EXX_OK;
 }
 
+// 5-D tensor map of W1 [t][q][pch][a][b2][pin] for pass C's tile gather: dimensions fastest first
+// (2 CHUNK doubles, R2, na, NPCH, R1 * max_batch), box = (2 CHUNK, 1, 1, NPCH, R1) = the whole tile of one transform, landing
+// dense (the layout the *_tg phase functions of exx_passes.cuh read).
+exx_status encode_w1_map(exx_plan* p, double2* w1, int max_batch, unsigned char out[128]) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                 const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap size");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(p, EXX_ERR_CUDA, "the driver does not provide cuTensorMapEncodeTiled");
+    }
+    int r1 = 0, r2 = 0;
+    bsplit_of(p->t[1], &r1, &r2);
+    const cuuint64_t chunk = static_cast<cuuint64_t>(p->geo.chunk), npch = static_cast<cuuint64_t>(p->t[2]) / chunk, na = static_cast<cuuint64_t>(p->n[0]);
+    const cuuint64_t dims[5] = {2 * chunk, static_cast<cuuint64_t>(r2), na, npch, static_cast<cuuint64_t>(r1) * max_batch};
+    const cuuint64_t strides[4] = {chunk * 16, r2 * chunk * 16, na * r2 * chunk * 16, npch * na * r2 * chunk * 16};
+    const cuuint32_t box[5] = {static_cast<cuuint32_t>(2 * chunk), 1, 1, static_cast<cuuint32_t>(npch), static_cast<cuuint32_t>(r1)};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    CUtensorMap map;
+    const CUresult r = reinterpret_cast<EncodeFn>(fn)(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, w1, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(p, EXX_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string(static_cast<int>(r)) + ")");
+    std::memcpy(out, &map, 128);
+    return EXX_OK;
+}
+
 // The new buffers are allocated BEFORE the old ones are released: a failed request (e.g. an absurd batch size) leaves
 // the plan exactly as it was, with its previous workspace and batch size.
 exx_status alloc_workspace(exx_plan* p, int max_batch) {
@@ -371,6 +402,12 @@ exx_status alloc_workspace(exx_plan* p, int max_batch) {
         cudaGetLastError();
         cudaFree(w1);
         return fail(p, EXX_ERR_ALLOC, "cudaMalloc(energy partials) failed; the previous workspace is kept");
+    }
+    if (p->info_c.needs_w1_map) {
+        unsigned char map[128];
+        const exx_status st = encode_w1_map(p, w1, max_batch, map);
+        if (st != EXX_OK) { cudaFree(w1); cudaFree(epart); return st; }
+        std::memcpy(p->w1_map, map, 128);
     }
     free_workspace(p);
     p->w1 = w1;
@@ -537,6 +574,9 @@ exx_status run_job_unguarded(exx_plan* p, const Job& job) {
     ArgsAC ac{};
     ac.psi = job.psi_str; ac.psi_r = job.psi_res; ac.kpsi = job.kpsi_str; ac.kpsi_r = job.kpsi_res;
     ac.w1 = p->w1; ac.twc = p->tw[2]; ac.twb = p->twb; ac.epart = p->epart;
+    ArgsCX cx{};
+    std::memcpy(cx.w1_map, p->w1_map, 128);
+    cx.twc_rot = p->twc_rot;
     ac.m_points = p->M; ac.na = p->n[0];
     ArgsB ab{};
     ab.w1 = p->w1; ab.twa = p->tw[0]; ab.ks = p->ks; ab.fullk = p->fullk; ab.tc = p->t[2];
@@ -562,9 +602,9 @@ exx_status run_job_unguarded(exx_plan* p, const Job& job) {
         if (job.psi_str_epi) {                             // Kernel 3 multiplies V[phi psi_i] with chi_i instead of psi_i
             ArgsAC acc = ac;
             acc.psi = job.psi_str_epi;
-            EXX_CUDA(p, launch_pass_c(p->geo, acc, s, nullptr));
+            EXX_CUDA(p, launch_pass_c(p->geo, acc, cx, s, nullptr));
         } else {
-            EXX_CUDA(p, launch_pass_c(p->geo, ac, s, nullptr));
+            EXX_CUDA(p, launch_pass_c(p->geo, ac, cx, s, nullptr));
         }
         EXX_CUDA(p, mark());
         p->launches += 3;
@@ -882,13 +922,33 @@ static exx_status create_impl(exx_plan** plan, const int dims[3], const double s
             return bail(fail(p, EXX_ERR_CUDA, "twiddle upload failed"));
         }
     }
+    {   // rotated c-axis twiddles (c1_compute_tg): class cls = (k1 = cls % PC, r = cls & 7), entry [n2*NCLS + cls] = W_TC^{n2 (k1 + PC r)}
+        int pc = 0, qc = 0;
+        split_of(p->t[2], &pc, &qc);
+        const int ncls = tg_classes(pc);
+        std::vector<double2> tw, roots, rot(static_cast<size_t>(qc) * ncls);
+        host_tables(p->t[2], tw, roots);
+        for (int n2 = 0; n2 < qc; ++n2)
+            for (int cls = 0; cls < ncls; ++cls) {
+                const long long m = static_cast<long long>(n2) * ((cls % pc) + pc * (cls & 7));
+                rot[static_cast<size_t>(n2) * ncls + cls] = roots[m % p->t[2]];
+            }
+        if (cudaMalloc(&p->twc_rot, rot.size() * sizeof(double2)) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(p, EXX_ERR_ALLOC, "cudaMalloc(twiddles) failed"));
+        }
+        if (cudaMemcpy(p->twc_rot, rot.data(), rot.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(p, EXX_ERR_CUDA, "twiddle upload failed"));
+        }
+    }
+
     exx_status st = build_fourier_kernel(p, kernel_host);
     if (st != EXX_OK) return bail(st);
 
     p->w1_elems_per_xform = static_cast<size_t>(p->n[0]) * p->t[1] * p->t[2];
     st = alloc_workspace(p, default_batch(p));
     if (st != EXX_OK) return bail(st);
-
     const size_t n = static_cast<size_t>(max_orbitals);
     p->desc_cap = max_transforms(n, n);
     bool ok = cudaMalloc(&p->e_mat, n * n * sizeof(double)) == cudaSuccess &&
@@ -948,6 +1008,7 @@ exx_status exx_plan_destroy(exx_plan* p) {
     }
     if (p->ks) cudaFree(p->ks);
     if (p->twb) cudaFree(p->twb);
+    if (p->twc_rot) cudaFree(p->twc_rot);
     free_workspace(p);
     if (p->e_mat) cudaFree(p->e_mat);
     if (p->occ_dev) cudaFree(p->occ_dev);

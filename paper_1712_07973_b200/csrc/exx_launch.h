@@ -22,6 +22,7 @@ struct KernelInfo {     // what a launcher reports about the instantiation it di
     int tiles;           // pass A / C: CTAs per launch (na * R2 / G);  pass B: blocks per transform (R1 * TC / CHUNK)
     int ctas_per_sm;     // occupancy the launcher sized its grid for (pass B: persistent grid = SMs * this)
     const char* name;    // kernel the launcher dispatches to for this geometry
+    int needs_w1_map;    // pass C: the kernel gathers its W1 tile through ArgsAC::w1_map (TMA tensor-box copy)
 };
 
 // Transform lengths the FFT covers.
@@ -36,7 +37,7 @@ const char* unsupported_geometry_text();
 // Each returns cudaSuccess or the launch/attribute error.  count = transforms in the batch.
 cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info);
 cudaError_t launch_pass_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info);
-cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info);
+cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, const ArgsCX& extra, cudaStream_t s, KernelInfo* info);
 // Query only (no launch): fills info for the geometry.
 cudaError_t query_pass_a(const Geometry& g, KernelInfo* info);
 cudaError_t query_pass_b(const Geometry& g, KernelInfo* info);

@@ -157,6 +157,15 @@ struct ArgsAC {
     double fj, fl;
     int count;                  // transforms in the batch
 };
+// Extra arguments of pass C's TMA-gather variant, a kernel parameter of their own: ArgsAC must not grow -- pass A at 256^3
+// free runs twice as long with 128 more bytes of kernel parameters (measured; same SASS up to register names).
+struct ArgsCX {
+    // CUtensorMap of W1 (5-D: [pin (2 CHUNK doubles)][b2][a][pch][q + R1 t]); opaque bytes here so that this header needs no
+    // driver types.  Valid only for the geometries whose pass C uses it (KernelInfo::needs_w1_map).
+    alignas(64) unsigned char w1_map[128];
+    const double2* twc_rot;     // [n2*NCLS + cls] = W_TC^{n2 (k1 + PC r)}, cls = k1-and-rotation class of a C1 item
+                                // (k1 = cls % PC, r = cls & 7, NCLS = lcm(8, PC)); see c1_compute_tg
+};
 
 // Offset (doubles) of real-space line l = gi*NB1 + b1 of tile (a, b2base) inside one orbital.
 template <class C>
@@ -340,6 +349,55 @@ EXX_HD void c2_compute(const double2* row, const XformDesc& d, int l, double fj,
     double xr[C::PC], xi[C::PC];
     c2_load<C>(row, xr, xi);
     c2_finish<C>(xr, xi, d, l, fj, fl, rj, rl, oi, accj, accl, e1, e2);
+}
+
+// ---- pass C with the TMA tile gather (TG).  ONE 5-D tensor-box copy brings the whole W1 tile of a transform; it lands
+//      dense and unpadded, rows q of TC elements (a tensor box cannot carry the bank-conflict padding of the layout above, and
+//      the hardware swizzles need a 128-byte contiguous inner dimension, which a 32-byte W1 run is not).  C0 and C2 run their
+//      lanes along a row and stay conflict-free; the lanes of C1 own one k1 segment each, 128 or 256 bytes apart, so lane
+//      item w reads and writes its segment ROTATED by r = w & 7 elements: at every step the 8 lanes of a quarter warp then
+//      touch 8 different bank groups.  An inverse DFT of the rotated input Y[j] = X[(j + r) mod QC] is the wanted output times
+//      a phase, x[n] = w_QC^{n r} IDFT(Y)[n], which together with the stage twiddle conj(W_TC^{n k1}) is conj(W_TC^{n (k1 + PC r)}):
+//      one table entry (ArgsCX::twc_rot, [n2][class], class = w mod lcm(8, PC)), so the rotation costs no arithmetic.  C1
+//      stores output n2 at position (n2 + r) mod QC of its segment, where C2 picks it up.
+//      Why: a cp.async gather writes shared memory sector by sector -- 17 to 24 wavefronts per warp instruction instead of
+//      4 -- and was the largest consumer of the shared-memory pipe in pass C.
+__host__ __device__ constexpr int tg_classes(int pc) { return pc % 8 == 0 ? pc : pc % 4 == 0 ? 2 * pc : pc % 2 == 0 ? 4 * pc : 8 * pc; }   // lcm(8, pc)
+template <class C>
+EXX_HD void c0_compute_tg(double2* col /* S + w */, const double2* tw) {
+    double xr[C::R1], xi[C::R1];
+#pragma unroll
+    for (int q = 0; q < C::R1; ++q) {
+        double2 v = col[q * C::TC];
+        xr[q] = v.x; xi[q] = v.y;
+        if (q > 0) cmul_conj(xr[q], xi[q], tw[q]);
+    }
+    dft_inv<C::R1, C::FREE>(xr, xi);
+#pragma unroll
+    for (int b1 = 0; b1 < C::NB1; ++b1) col[b1 * C::TC] = make_double2(xr[b1], xi[b1]);
+}
+// seg = S + line*TC + k1*QC; r = item & 7; tw = twc_rot + class, stride tws = number of classes
+template <class C>
+EXX_HD void c1_compute_tg(double2* seg, int r, const double2* tw, int tws) {
+    static_assert(C::QC == 8 || C::QC == 16, "the rotation needs a power-of-two segment of at least 8 elements");
+    double xr[C::QC], xi[C::QC];
+#pragma unroll
+    for (int j = 0; j < C::QC; ++j) { double2 v = seg[(j + r) & (C::QC - 1)]; xr[j] = v.x; xi[j] = v.y; }
+    dft_inv<C::QC, false>(xr, xi);
+#pragma unroll
+    for (int n2 = 0; n2 < C::QC; ++n2) {
+        cmul_conj(xr[n2], xi[n2], tw[n2 * tws]);
+        seg[(n2 + r) & (C::QC - 1)] = make_double2(xr[n2], xi[n2]);
+    }
+}
+// row = S + line*TC; the element n2 of segment k1 of line `line` sits at position (n2 + ((line*PC + k1) & 7)) mod QC
+template <class C>
+EXX_HD void c2_load_tg(const double2* row, int line, int n2, double* xr /*[PC]*/, double* xi /*[PC]*/) {
+#pragma unroll
+    for (int k1 = 0; k1 < C::PC; ++k1) {
+        double2 v = row[k1 * C::QC + ((n2 + ((line * C::PC + k1) & 7)) & (C::QC - 1))];
+        xr[k1] = v.x; xi[k1] = v.y;
+    }
 }
 
 // ---------------------------------------------------------------------------------------- pass B geometry
@@ -1126,17 +1184,31 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
 //     deterministic.
 //   * EARLY (single work buffer only): C2 first takes its inputs into registers, which frees the buffer, and the gather
 //     of transform t+1 is issued from there, so that its latency hides behind the P-point stage and the epilogue of t.
+//   * TG (single work buffer, one b2 per tile, rows of a multiple of 64 elements): the tile arrives by ONE TMA tensor-box
+//     copy issued by thread 0 (mbarrier completion) instead of R1 cp.async per column, in the swizzled dense layout of
+//     the *_tg phase functions.
+template <class C, int NBUF>
+__host__ __device__ constexpr bool pass_c_tma_gather() {
+#ifdef EXX_NO_TG
+    return false;
+#else
+    return C::G == 1 && C::TC % 64 == 0 && NBUF == 1;
+#endif
+}
 template <class C, int NT, int NSTG, int NBUF, int MINB, bool EARLY>
-__global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
+__global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g, const __grid_constant__ ArgsCX gx) {
     static_assert(!EARLY || NBUF == 1, "the early gather is the single-buffer scheme");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2* const S0 = reinterpret_cast<double2*>(smem_raw);
+    constexpr bool TG = pass_c_tma_gather<C, NBUF>();
+    extern __shared__ __align__(128) unsigned char smem_raw_c[];        // tensor-box destination: 128-byte aligned
+    double2* const S0 = reinterpret_cast<double2*>(smem_raw_c);
     double* const OP = reinterpret_cast<double*>(S0 + NBUF * C::SMEM_C);
     double* const RES = OP + NSTG * C::OP_DOUBLES;
     __shared__ uint64_t full[NSTG];
-    __shared__ uint64_t resbar;
+    __shared__ uint64_t resbar, gbar;
     __shared__ double red[2][NT / 32];
-    __shared__ double2 s_twct[C::TC], s_twb[C::TB];        // twiddle tables; the c-axis one transposed to [n2*PC + k1]
+    constexpr int NCLS = tg_classes(C::PC);
+    __shared__ double2 s_twct[TG ? C::QC * NCLS : C::TC], s_twb[C::TB];   // twiddle tables; the c-axis one transposed to [n2*PC + k1]
+                                                                          // (TG: the rotated one, [n2*NCLS + class])
     const int tile = blockIdx.x, tid = threadIdx.x;
     const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
     constexpr int NI0 = ceil_div(C::ITEMS_POS, NT), NI1 = ceil_div(C::ITEMS_LINE_P, NT), NI2 = ceil_div(C::ITEMS_LINE_Q, NT);
@@ -1144,9 +1216,11 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     if (tid == 0) {
         for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
         mbar_init(&resbar, 1);
+        mbar_init(&gbar, 1);
         mbar_fence_init();
     }
-    for (int x = tid; x < C::TC; x += NT) s_twct[(x % C::QC) * C::PC + x / C::QC] = g.twc[x];
+    if (TG) { for (int x = tid; x < C::QC * NCLS; x += NT) s_twct[x] = gx.twc_rot[x]; }
+    else { for (int x = tid; x < C::TC; x += NT) s_twct[(x % C::QC) * C::PC + x / C::QC] = g.twc[x]; }
     for (int x = tid; x < C::TB; x += NT) s_twb[x] = g.twb[x];
     __syncthreads();
 
@@ -1155,6 +1229,14 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
     for (int m = 0; m < NI0; ++m) c0[m] = col_index<C, true>(tid + m * NT < C::ITEMS_POS ? tid + m * NT : 0, a, b2base, g.na);
     const size_t qstride = C::w1_q(g.na), tstride = C::w1_t(g.na);
     auto issue_w1_gather = [&](int t) {
+        if (TG) {                                          // one tensor box: (pin, b2, a, all pch, the R1 q-rows of transform t)
+            if (tid == 0) {
+                fence_proxy_async();                       // the buffer was last written by generic stores (C0 / C1 of t-1)
+                mbar_arrive_expect_tx(&gbar, C::R1 * C::TC * 16);
+                tensor5_g2s(S0, gx.w1_map, 0, b2base, a, 0, t * C::R1, &gbar);
+            }
+            return;
+        }
         double2* dstbuf = S0 + (NBUF == 2 ? (t & 1) : 0) * C::SMEM_C;
         const double2* w1t = g.w1 + static_cast<size_t>(t) * tstride;
 #pragma unroll
@@ -1208,15 +1290,18 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             cp_async_commit();
             cp_async_wait<1>();                            // this thread's columns of transform t have landed
         } else if (EARLY) {                                // single work buffer, gather of t issued from inside C2 of t-1
-            cp_async_wait<0>();
+            if (TG) mbar_wait(&gbar, t & 1); else cp_async_wait<0>();
         } else {                                           // single work buffer: no overlap of the gather
             issue_w1_gather(t);
             cp_async_commit();
-            cp_async_wait<0>();
+            if (TG) mbar_wait(&gbar, t & 1); else cp_async_wait<0>();
         }
 #pragma unroll
         for (int m = 0; m < NI0; ++m)
-            if (tid + m * NT < C::ITEMS_POS) c0_compute<C>(S + c0[m].col, s_twb + c0[m].b2 * C::R1);
+            if (tid + m * NT < C::ITEMS_POS) {
+                if constexpr (TG) c0_compute_tg<C>(S + tid + m * NT, s_twb + c0[m].b2 * C::R1);
+                else c0_compute<C>(S + c0[m].col, s_twb + c0[m].b2 * C::R1);
+            }
         if (DEFER && tid < 32 && refill_t >= 0) {
             bulk_wait_read_all();                          // the stage may be overwritten
             __syncwarp();
@@ -1226,7 +1311,10 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
         __syncthreads();
 #pragma unroll
         for (int m = 0; m < NI1; ++m)
-            if (tid + m * NT < C::ITEMS_LINE_P) c1_compute<C>(S + p1[m].seg, s_twct + p1[m].k1, C::PC, p1[m].k1);
+            if (tid + m * NT < C::ITEMS_LINE_P) {
+                if constexpr (TG) c1_compute_tg<C>(S + ((tid + m * NT) / C::PC) * C::TC + p1[m].k1 * C::QC, (tid + m * NT) & 7, s_twct + (tid + m * NT) % NCLS, NCLS);
+                else c1_compute<C>(S + p1[m].seg, s_twct + p1[m].k1, C::PC, p1[m].k1);
+            }
         __syncthreads();
         double e1 = 0.0, e2 = 0.0;
         if (!EARLY) {
@@ -1234,9 +1322,17 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             mbar_wait(&full[s], (t / NSTG) & 1);           // psi_i lines of transform t have landed
 #pragma unroll
             for (int m = 0; m < NI2; ++m)
-                if (tid + m * NT < C::ITEMS_LINE_Q)
-                    c2_compute<C>(S + q2[m].row, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
-                                  accj[m], accl[m], e1, e2);
+                if (tid + m * NT < C::ITEMS_LINE_Q) {
+                    if constexpr (TG) {
+                        double xr[C::PC], xi[C::PC];
+                        c2_load_tg<C>(S + ((tid + m * NT) / C::QC) * C::TC, (tid + m * NT) / C::QC, q2[m].n2, xr, xi);
+                        c2_finish<C>(xr, xi, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                                     accj[m], accl[m], e1, e2);
+                    } else {
+                        c2_compute<C>(S + q2[m].row, d, g.ld, g.fj, g.fl, RES + q2[m].op, RES + C::LINES * C::LS + q2[m].op, stage + q2[m].op,
+                                      accj[m], accl[m], e1, e2);
+                    }
+                }
         } else {
             // single work buffer: every item first takes its inputs into registers; after the barrier nothing of transform
             // t is left in the buffer, so the W1 tile of t+1 is gathered into it while the P-point stage and the Kernel-3
@@ -1244,7 +1340,10 @@ __global__ void __launch_bounds__(NT, MINB) pass_c_kernel(const ArgsAC g) {
             double xr[NI2][C::PC], xi[NI2][C::PC];
 #pragma unroll
             for (int m = 0; m < NI2; ++m)
-                if (tid + m * NT < C::ITEMS_LINE_Q) c2_load<C>(S + q2[m].row, xr[m], xi[m]);
+                if (tid + m * NT < C::ITEMS_LINE_Q) {
+                    if constexpr (TG) c2_load_tg<C>(S + ((tid + m * NT) / C::QC) * C::TC, (tid + m * NT) / C::QC, q2[m].n2, xr[m], xi[m]);
+                    else c2_load<C>(S + q2[m].row, xr[m], xi[m]);
+                }
             __syncthreads();
             if (t + 1 < g.count) issue_w1_gather(t + 1);
             cp_async_commit();

@@ -33,7 +33,7 @@ def _build():
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
     if not os.path.exists(nvcc):
         pytest.skip("nvcc not available")
-    subprocess.run([nvcc, "-std=c++17", "-O1", "-x", "cu", "-Wno-deprecated-gpu-targets", "-Xcompiler", "-fPIC", "-shared",
+    subprocess.run([nvcc, "-std=c++17", "-O1", "-x", "cu", "-arch=sm_100a", "-Wno-deprecated-gpu-targets", "-Xcompiler", "-fPIC", "-shared",
                     "-I", CSRC, "-o", LIB, SRC], check=True)
     return LIB
 
