@@ -151,7 +151,8 @@ def test_warp_specialised_kernels_edge_schedule(base, dims):
 
 
 @pytest.mark.parametrize("base,dims,n_orb,batch", [("C1", (32, 32, 32), 5, 2), ("C1", (96, 96, 96), 5, 3), ("C2", (48, 48, 48), 4, 0),
-                                                   ("C1", (192, 96, 48), 3, 2), ("C2", (16, 64, 32), 3, 0)])
+                                                   ("C1", (192, 96, 48), 3, 2), ("C2", (16, 64, 32), 3, 0),
+                                                   ("C1", (192, 192, 192), 3, 2), ("C2", (128, 128, 128), 2, 0)])   # TMA tile gather
 def test_guard_bands_and_poisoned_outputs(base, dims, n_orb, batch):
     """Memory-safety evidence that needs no tool (compute-sanitizer is closed on this pool): psi and K psi live in the
     middle of larger allocations whose guard bands hold a sentinel, K psi starts as NaN, and E_x / e_ij start as NaN.
