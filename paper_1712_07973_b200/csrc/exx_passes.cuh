@@ -1019,6 +1019,12 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
     constexpr int NT = 32 * (NY + NX), NXT = 32 * NX;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     constexpr int NQ = ceil_div(C::ITEMS_Q, 32), NP = ceil_div(C::ITEMS_P, 32), NIO = ceil_div(C::ITEMS_IO, NXT);
+    // ROWST: B4 writes its result back into the rows and every row leaves by one TMA bulk store.  A direct B4 store is a
+    // scattered 16-byte STG whose warp instruction touches 32 / CHUNK different 32 * CHUNK-byte runs: with CHUNK = 2 that is one
+    // LSU wavefront per 32-byte sector, 16 per instruction, where the in-place shared-memory store costs 4 (the LSU data
+    // pipe of pass B stood at 82 %).  Measured: pass B -11 % at 256^3 free, -3 % at 192^3; with CHUNK = 4 (64-byte runs, 96^3)
+    // the direct stores are cheap enough and the extra shared-memory round trip loses (+12 %).
+    constexpr bool ROWST = C::CHUNK <= 2;
 
     if (tid == 0) {
         for (int b = 0; b < 2; ++b) { mbar_init(&full[b], NX); mbar_init(&ready[b], NX); mbar_init(&done[b], NY); }
@@ -1076,12 +1082,33 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
             double2* const W = BUF + (k & 1) * BUF_ELEMS;
             double2* blk = block_ptr(id0 + k * stride);
             mbar_wait(&done[k & 1], (k >> 1) & 1);
+            if constexpr (ROWST) {
+                // B4 back into the rows (in place), then one TMA bulk store per row
 #pragma unroll
-            for (int m = 0; m < NIO; ++m)
-                if (xt + m * NXT < C::ITEMS_IO) {
-                    const IoIdx x = io_index<C>(xt + m * NXT);
-                    b4_compute<C>(W + x.s, blk + x.g);
+                for (int m = 0; m < NIO; ++m)
+                    if (xt + m * NXT < C::ITEMS_IO) {
+                        const IoIdx x = io_index<C>(xt + m * NXT);
+                        b4_compute<C>(W + x.s, W + x.s);
+                    }
+                fence_proxy_async();                       // generic-proxy writes of the rows precede the TMA reads
+                __syncwarp();
+#pragma unroll
+                for (int m = 0; m < NIO; ++m) {
+                    const int idx = xt + m * NXT;
+                    if (idx < C::ITEMS_IO && idx % C::CHUNK == 0) {
+                        const int a = idx / C::CHUNK;
+                        bulk_s2g(blk + a * C::COLS, W + C::row_off(a), C::ROW_BYTES);
+                    }
                 }
+                bulk_commit();
+            } else {
+#pragma unroll
+                for (int m = 0; m < NIO; ++m)
+                    if (xt + m * NXT < C::ITEMS_IO) {
+                        const IoIdx x = io_index<C>(xt + m * NXT);
+                        b4_compute<C>(W + x.s, blk + x.g);
+                    }
+            }
         };
         if (nk > 0) issue_row_loads(0);
         if (nk > 1) issue_row_loads(1);
@@ -1099,6 +1126,7 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
             if (k >= 1) {
                 b4_block(k - 1);
                 if (k + 1 < nk) {
+                    if (ROWST) bulk_wait_read_all();       // the row stores of block k-1 have read their rows
                     fence_proxy_async();                   // this warp's reads of its rows precede the TMA writes
                     __syncwarp();
                     issue_row_loads(k + 1);
@@ -1106,6 +1134,7 @@ __global__ void __launch_bounds__(32 * (NY + NX), MINB) pass_b_ws_kernel(const A
             }
         }
         if (nk > 0) b4_block(nk - 1);
+        if (ROWST) bulk_wait_all();                        // shared memory must outlive the row stores
     } else {
         // ------------------------------------------------------------------ column warps: a-axis phases
         // K^ of this lane's B2 item (one item per lane, NP = 1) is requested ahead of B1 so that the L2 latency hides
