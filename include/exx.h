@@ -275,6 +275,26 @@ exx_status exx_diag_fp64(void *cuda_stream, double *dfma_tflops, double *dadd_to
  */
 exx_status exx_diag_shfl(void *cuda_stream, double *shfl_gbs, double *shfl_lds_overlap);
 
+/*
+ * exx_exchange_energy_noalloc -- the ONE entry point that allocates nothing (no cudaMalloc / cudaFree / allocating library
+ * call, no plan): for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it).  It evaluates the operator form of the exchange energy (Eq. 5 with Eq. 3 inserted),
+ *      E_x = 1/2 dV sum_i f_i sum_r psi_i(r) (K psi)_i(r),
+ * from the orbitals and the K psi an exx_apply* call produced, with a fixed-order (deterministic) two-stage reduction whose
+ * scratch -- 1024 per-block partial sums and the device copy of the occupations -- is a file-scope static __device__ array of
+ * 40 KB that every GPU loading the library holds until exit (csrc/exx_noalloc.cu).
+ *   n_orb     <= EXX_NOALLOC_MAX_ORBITALS, else EXX_ERR_UNSUPPORTED_SIZE (text from exx_noalloc_last_error);
+ *   n_points  n1*n2*n3;  dV = h1*h2*h3;  psi_dev, kpsi_dev DEVICE [n_orb][n_points], read-only;  occ_host HOST [n_orb];
+ *   ex_dev    DEVICE, one double, written on cuda_stream (NULL = default stream).  Does not synchronise.
+ * Runs on the CURRENT device.  All calls share the static scratch, which keeps the previous call's contents (nothing in it
+ * has to start at zero: every slot that is read is written earlier in the same call); calls on one stream are ordered, calls
+ * that OVERLAP on the GPU (other streams / threads) race on it.
+ */
+#define EXX_NOALLOC_MAX_ORBITALS 4096
+exx_status  exx_exchange_energy_noalloc(int n_orb, long long n_points, double dV, const double *psi_dev, const double *kpsi_dev,
+                                        const double *occ_host, double *ex_dev, void *cuda_stream);
+const char *exx_noalloc_last_error(void);           /* per host thread; "" after a successful call */
+
 exx_status  exx_plan_destroy(exx_plan *plan);       /* NULL is allowed */
 const char *exx_status_string(exx_status s);
 const char *exx_last_error(const exx_plan *plan);   /* detail text incl. CUDA error name; plan may be NULL for

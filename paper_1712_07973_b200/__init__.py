@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     exx_apply,
     exx_diag_fp64,
     exx_diag_shfl,
+    exx_exchange_energy_noalloc,
     exx_plan_create,
     exx_plan_destroy,
     exx_round_robin_step,

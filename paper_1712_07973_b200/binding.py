@@ -28,6 +28,7 @@ EXPORTS = [
     "exx_schedule_pairs", "exx_schedule_list", "exx_schedule_list_masked", "exx_schedule_list_block", "exx_round_robin_step",
     "exx_plan_transform_dims", "exx_plan_workspace_bytes", "exx_plan_launch_count", "exx_plan_device", "exx_plan_kernel_name",
     "exx_plan_set_batch", "exx_plan_set_profiling", "exx_plan_get_profile", "exx_plan_destroy", "exx_status_string", "exx_last_error", "exx_version", "exx_diag_fp64", "exx_diag_shfl",
+    "exx_exchange_energy_noalloc", "exx_noalloc_last_error",
 ]
 
 _lib = None
@@ -115,6 +116,10 @@ def load_library():
     lib.exx_diag_fp64.restype = C.c_int
     lib.exx_diag_shfl.argtypes = [C.c_void_p, _dp, _dp]
     lib.exx_diag_shfl.restype = C.c_int
+    lib.exx_exchange_energy_noalloc.argtypes = [C.c_int, C.c_longlong, C.c_double, C.c_void_p, C.c_void_p, _dp, C.c_void_p, C.c_void_p]
+    lib.exx_exchange_energy_noalloc.restype = C.c_int
+    lib.exx_noalloc_last_error.argtypes = []
+    lib.exx_noalloc_last_error.restype = C.c_char_p
     lib.exx_version.argtypes = []
     lib.exx_version.restype = C.c_char_p
     _lib = lib
@@ -141,6 +146,29 @@ def exx_diag_shfl(stream: Optional[int] = None) -> dict:
     if st:
         raise ExxError(st, "exx_diag_shfl")
     return {"shfl_gbs": v[0].value, "shfl_lds_overlap": v[1].value}
+
+
+EXX_NOALLOC_MAX_ORBITALS = 4096
+
+
+def exx_exchange_energy_noalloc(psi, kpsi, occ, dV: float, ex_dev, stream: Optional[int] = None) -> None:
+    """include/exx.h exx_exchange_energy_noalloc: E_x = 1/2 dV sum_i f_i <psi_i|K psi_i> into ex_dev (CUDA fp64, 1 element), with
+    no allocation anywhere (static device scratch; calls that overlap on the GPU race on it).  Does not synchronise."""
+    import torch
+    for name, t in (("psi", psi), ("kpsi", kpsi), ("ex_dev", ex_dev)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA float64 tensor")
+    if psi.shape != kpsi.shape or psi.dim() < 2 or ex_dev.numel() < 1:
+        raise ValueError("psi and kpsi must have the same shape (N, ...) and ex_dev at least one element")
+    n_orb = int(psi.shape[0])
+    occ = np.ascontiguousarray(np.asarray(occ, dtype=np.float64))
+    if occ.ndim != 1 or occ.size != n_orb:
+        raise ValueError(f"occ must hold one occupation per orbital ({n_orb})")
+    lib = load_library()
+    st = lib.exx_exchange_energy_noalloc(n_orb, psi[0].numel(), float(dV), C.c_void_p(psi.data_ptr()), C.c_void_p(kpsi.data_ptr()),
+                                         occ.ctypes.data_as(_dp), C.c_void_p(ex_dev.data_ptr()), C.c_void_p(stream) if stream else None)
+    if st:
+        raise ExxError(st, lib.exx_noalloc_last_error().decode())
 
 
 def exx_schedule_pairs(occ: Sequence[float]):

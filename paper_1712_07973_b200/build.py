@@ -22,7 +22,8 @@ if DEV:
 MODE = "dev:" + ",".join(map(str, TB_LENGTHS)) if DEV else "full"
 # (source, extra defines, object name); the heaviest units first so that the parallel build ends sooner
 UNITS = [(f"exx_pass_{p}.cu", [f"-DEXX_TB={tb}"], f"exx_pass_{p}_{tb}.o") for tb in reversed(TB_LENGTHS) for p in "bca"] + \
-        [("exx_api.cu", [], "exx_api.o"), ("exx_dispatch.cu", [], "exx_dispatch.o"), ("exx_diag.cu", [], "exx_diag.o")]
+        [("exx_api.cu", [], "exx_api.o"), ("exx_dispatch.cu", [], "exx_dispatch.o"), ("exx_diag.cu", [], "exx_diag.o"),
+         ("exx_noalloc.cu", [], "exx_noalloc.o")]
 SOURCES = sorted({u[0] for u in UNITS})
 HEADERS = ["exx_dft.cuh", "exx_async.cuh", "exx_passes.cuh", "exx_launch.h", "exx_inst.cuh", "exx_sched.hpp", "../../include/exx.h"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
