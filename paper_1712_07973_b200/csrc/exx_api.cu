@@ -403,7 +403,7 @@ exx_status alloc_workspace(exx_plan* p, int max_batch) {
         cudaFree(w1);
         return fail(p, EXX_ERR_ALLOC, "cudaMalloc(energy partials) failed; the previous workspace is kept");
     }
-    if (p->info_c.needs_w1_map) {
+    if (p->info_a.needs_w1_map || p->info_c.needs_w1_map) {
         unsigned char map[128];
         const exx_status st = encode_w1_map(p, w1, max_batch, map);
         if (st != EXX_OK) { cudaFree(w1); cudaFree(epart); return st; }
@@ -595,7 +595,7 @@ exx_status run_job_unguarded(exx_plan* p, const Job& job) {
         ac.jd = job.square ? b.j : -1;
         ac.ld = job.square ? b.l : -2;
         EXX_CUDA(p, mark());
-        EXX_CUDA(p, launch_pass_a(p->geo, ac, s, nullptr));
+        EXX_CUDA(p, launch_pass_a(p->geo, ac, cx, s, nullptr));
         EXX_CUDA(p, mark());
         EXX_CUDA(p, launch_pass_b(p->geo, ab, b.count, s, nullptr));
         EXX_CUDA(p, mark());

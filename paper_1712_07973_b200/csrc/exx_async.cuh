@@ -62,6 +62,13 @@ __device__ __forceinline__ void tensor5_g2s(void* dst_smem, const void* tensor_m
                  : "memory");
 }
 
+// 5-D tensor-box store shared -> global through a CUtensorMap (bulk async-group completion)
+__device__ __forceinline__ void tensor5_s2g(const void* tensor_map, int c0, int c1, int c2, int c3, int c4, const void* src_smem) {
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1, %2, %3, %4, %5}], [%6];"
+                 ::"l"(tensor_map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src_smem))
+                 : "memory");
+}
+
 // shared -> global plain store / fp64 reduce-add (bulk async-group completion)
 __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes)

@@ -6,15 +6,15 @@
 namespace exx {
 
 #define X(T)                                                                                                                           \
-    bool try_pass_a_##T(const Geometry&, const ArgsAC&, cudaStream_t, KernelInfo*, bool, cudaError_t*);                                \
+    bool try_pass_a_##T(const Geometry&, const ArgsAC&, const ArgsCX&, cudaStream_t, KernelInfo*, bool, cudaError_t*);                                \
     bool try_pass_b_##T(const Geometry&, const ArgsB&, int, cudaStream_t, KernelInfo*, bool, cudaError_t*);                            \
     bool try_pass_c_##T(const Geometry&, const ArgsAC&, const ArgsCX&, cudaStream_t, KernelInfo*, bool, cudaError_t*);
 EXX_ALL_LENGTHS(X)
 #undef X
 
-static cudaError_t dispatch_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info, bool launch) {
+static cudaError_t dispatch_a(const Geometry& g, const ArgsAC& args, const ArgsCX& extra, cudaStream_t s, KernelInfo* info, bool launch) {
     cudaError_t err = cudaErrorInvalidValue;
-#define X(T) if (try_pass_a_##T(g, args, s, info, launch, &err)) return err;
+#define X(T) if (try_pass_a_##T(g, args, extra, s, info, launch, &err)) return err;
     EXX_ALL_LENGTHS(X)
 #undef X
     return cudaErrorInvalidValue;
@@ -34,14 +34,15 @@ static cudaError_t dispatch_c(const Geometry& g, const ArgsAC& args, const ArgsC
     return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info) { return dispatch_a(g, args, s, info, true); }
+cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, const ArgsCX& extra, cudaStream_t s, KernelInfo* info) { return dispatch_a(g, args, extra, s, info, true); }
 cudaError_t launch_pass_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info) { return dispatch_b(g, args, count, s, info, true); }
 cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, const ArgsCX& extra, cudaStream_t s, KernelInfo* info) { return dispatch_c(g, args, extra, s, info, true); }
 
 cudaError_t query_pass_a(const Geometry& g, KernelInfo* info) {
     ArgsAC args{};
     args.na = g.free_bc ? g.ta / 2 : g.ta;
-    return dispatch_a(g, args, nullptr, info, false);
+    ArgsCX extra{};
+    return dispatch_a(g, args, extra, nullptr, info, false);
 }
 cudaError_t query_pass_b(const Geometry& g, KernelInfo* info) {
     ArgsB args{};

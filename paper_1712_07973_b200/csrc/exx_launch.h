@@ -22,7 +22,7 @@ struct KernelInfo {     // what a launcher reports about the instantiation it di
     int tiles;           // pass A / C: CTAs per launch (na * R2 / G);  pass B: blocks per transform (R1 * TC / CHUNK)
     int ctas_per_sm;     // occupancy the launcher sized its grid for (pass B: persistent grid = SMs * this)
     const char* name;    // kernel the launcher dispatches to for this geometry
-    int needs_w1_map;    // pass C: the kernel gathers its W1 tile through ArgsAC::w1_map (TMA tensor-box copy)
+    int needs_w1_map;    // passes A / C: the kernel moves its W1 tile through ArgsCX::w1_map (TMA tensor-box store / copy)
 };
 
 // Transform lengths the FFT covers.
@@ -35,7 +35,7 @@ int chunk_of(const Geometry& g);
 const char* unsupported_geometry_text();
 
 // Each returns cudaSuccess or the launch/attribute error.  count = transforms in the batch.
-cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, cudaStream_t s, KernelInfo* info);
+cudaError_t launch_pass_a(const Geometry& g, const ArgsAC& args, const ArgsCX& extra, cudaStream_t s, KernelInfo* info);
 cudaError_t launch_pass_b(const Geometry& g, const ArgsB& args, int count, cudaStream_t s, KernelInfo* info);
 cudaError_t launch_pass_c(const Geometry& g, const ArgsAC& args, const ArgsCX& extra, cudaStream_t s, KernelInfo* info);
 // Query only (no launch): fills info for the geometry.
@@ -191,6 +191,14 @@ struct TuneAC {
         (2 * CfgA::SMEM_A * 16 + 1 * CfgA::OP_DOUBLES * 8 + kStaticA) * 2 <= kSmemPerSM + 1024 ? 1 : 2;
     static constexpr int SMEM_A_WS = 2 * CfgA::SMEM_A * 16 + NSTG_A_WS * CfgA::OP_DOUBLES * 8;
     static constexpr int MINB_A_WS = pick_minb(SMEM_A_WS + kStaticA, 32 * (NAW + NBW), 96, 2, CfgA::NC * CfgA::TILES_PER_A);
+    // ---- pass A with the TMA tile store (pass_a_ts_kernel): two dense R1 x TC work buffers
+    static constexpr int kBufTS = BSplit<TB>::R1 * TC * 16;
+    static constexpr int NSTG_A_TS =
+        (2 * kBufTS + 2 * CfgA::OP_DOUBLES * 8 + kStaticA) * 2 <= kSmemPerSM + 1024 ? 2 :
+        (2 * kBufTS + 1 * CfgA::OP_DOUBLES * 8 + kStaticA) * 2 <= kSmemPerSM + 1024 ? 1 : 2;
+    static constexpr int SMEM_A_TS = 2 * kBufTS + NSTG_A_TS * CfgA::OP_DOUBLES * 8;
+    static constexpr int MINB_A_TS = pick_minb(SMEM_A_TS + kStaticA, 32 * (NAW + NBW), 96, 2, CfgA::NC * CfgA::TILES_PER_A);
+    static constexpr bool TS_A = WS_A && pass_a_tma_store<CfgA>() && SMEM_A_TS <= kMaxSmemAC;
     static_assert(SMEM_C <= kMaxSmemAC && SMEM_A <= kMaxSmemAC && SMEM_A_WS <= kMaxSmemAC, "tile does not fit shared memory");
 };
 

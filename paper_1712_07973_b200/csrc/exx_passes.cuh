@@ -400,6 +400,68 @@ EXX_HD void c2_load_tg(const double2* row, int line, int n2, double* xr /*[PC]*/
     }
 }
 
+// ---- pass A with the TMA tile store (TS), the mirror of the gather above: the (R1 x TC) output tile of a transform leaves by
+//      ONE tensor-box store out of a dense shared-memory tile, rows of TC elements, instead of R1 scattered 16-byte stores
+//      per column (32-byte runs in W1: one LSU wavefront per sector, 16 per warp instruction; the LSU data pipe of pass A stood
+//      at 87 % at 192^3).  The work buffer is that dense tile; A0 stores, and A1 works on, every k1 segment ROTATED by
+//      r = (line*PC + k1) & 7 elements (element n2 / k2 of the segment sits at position (index + r) mod QC), which keeps the
+//      segment-per-lane accesses of A1 conflict-free without padding; A2 reads through the rotation and writes its R1 outputs
+//      in place at the natural position.  Pure address arithmetic: no phase enters (unlike C1, where the rotation is applied to
+//      the transform's input order).
+template <class C>
+EXX_HD int ts_pos(int line, int k1, int i) { return k1 * C::QC + ((i + ((line * C::PC + k1) & 7)) & (C::QC - 1)); }
+template <class C>
+EXX_HD void a0_compute_ts(const double* vj, const double* vl, const double* pi, int flags, double2* row /* S + line*TC */, int line, int n2,
+                          const double2* tw /* twc + n2 */) {
+    double xr[C::PC], xi[C::PC];
+#pragma unroll
+    for (int n1 = 0; n1 < C::PCN; ++n1) {
+        const double p = pi[C::QC * n1];
+        xr[n1] = vj[n1] * p;
+        xi[n1] = vl[n1] * p;
+    }
+    if (flags != 3) {
+        const double m1 = (flags & 1) ? 1.0 : 0.0, m2 = (flags & 2) ? 1.0 : 0.0;
+#pragma unroll
+        for (int n1 = 0; n1 < C::PCN; ++n1) { xr[n1] *= m1; xi[n1] *= m2; }
+    }
+#pragma unroll
+    for (int n1 = C::PCN; n1 < C::PC; ++n1) { xr[n1] = 0.0; xi[n1] = 0.0; }
+    dft_fwd<C::PC, C::FREE>(xr, xi);
+#pragma unroll
+    for (int k1 = 0; k1 < C::PC; ++k1) {
+        if (k1 > 0) cmul(xr[k1], xi[k1], tw[k1 * C::QC]);
+        row[ts_pos<C>(line, k1, n2)] = make_double2(xr[k1], xi[k1]);
+    }
+}
+template <class C>
+EXX_HD void a1_compute_ts(double2* seg /* S + line*TC + k1*QC */, int r) {
+    double xr[C::QC], xi[C::QC];
+#pragma unroll
+    for (int n2 = 0; n2 < C::QC; ++n2) { double2 v = seg[(n2 + r) & (C::QC - 1)]; xr[n2] = v.x; xi[n2] = v.y; }
+    Dft<C::QC>::run(xr, xi);
+#pragma unroll
+    for (int k2 = 0; k2 < C::QC; ++k2) seg[(k2 + r) & (C::QC - 1)] = make_double2(xr[k2], xi[k2]);
+}
+// column p = k1*QC + k2 of the tile: loads (through the rotation), transform, then -- after the caller's __syncwarp, since
+// another lane of the warp may still have to read the element this one overwrites -- a2_store_ts
+template <class C>
+EXX_HD void a2_load_ts(const double2* S, int k1, int k2, double* xr /*[R1]*/, double* xi /*[R1]*/) {
+#pragma unroll
+    for (int b1 = 0; b1 < C::NB1; ++b1) { double2 v = S[b1 * C::TC + ts_pos<C>(b1, k1, k2)]; xr[b1] = v.x; xi[b1] = v.y; }
+#pragma unroll
+    for (int b1 = C::NB1; b1 < C::R1; ++b1) { xr[b1] = 0.0; xi[b1] = 0.0; }
+}
+template <class C>
+EXX_HD void a2_store_ts(double* xr, double* xi, const double2* tw /* twb + b2*R1 */, double2* col /* S + p */) {
+    dft_fwd<C::R1, C::FREE>(xr, xi);
+#pragma unroll
+    for (int q = 0; q < C::R1; ++q) {
+        if (q > 0) cmul(xr[q], xi[q], tw[q]);
+        col[q * C::TC] = make_double2(xr[q], xi[q]);
+    }
+}
+
 // ---------------------------------------------------------------------------------------- pass B geometry
 // Shared-memory bank model for 16-byte accesses: a warp request is served quarter-warp by quarter-warp (8 lanes,
 // 128 bytes); lanes of a quarter that hit the same 16-byte bank group (offset mod 8) at different addresses
@@ -907,6 +969,117 @@ __global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_a_ws_kernel(const
             __syncwarp();
             if (lane == 0) mbar_arrive(&sfree[b]);
         }
+    }
+}
+
+// Pass A with the TMA tile store (see the *_ts phase functions): the warp-specialised structure of pass_a_ws_kernel with dense
+// R1 x TC work buffers.  The column warps run A2 in place, synchronise among themselves, and one thread sends the tile out
+// with a tensor-box store; the buffer goes back to the line warps once the store has READ it.
+template <class C>
+__host__ __device__ constexpr bool pass_a_tma_store() {
+#ifdef EXX_NO_TS
+    return false;
+#else
+    return C::G == 1 && C::TC % 64 == 0 && (C::QC == 8 || C::QC == 16) && !C::FREE;
+#endif
+}
+template <class C, int NAW, int NBW, int NSTG, int MINB>
+__global__ void __launch_bounds__(32 * (NAW + NBW), MINB) pass_a_ts_kernel(const ArgsAC g, const __grid_constant__ ArgsCX gx) {
+    extern __shared__ __align__(128) unsigned char smem_raw_a[];
+    constexpr int BUF = C::R1 * C::TC;                                   // one dense work buffer = one W1 tile
+    double2* const S0 = reinterpret_cast<double2*>(smem_raw_a);
+    double* const OP = reinterpret_cast<double*>(S0 + 2 * BUF);
+    __shared__ uint64_t full[NSTG], sready[2], sfree[2];
+    __shared__ double2 s_twc[C::TC], s_twb[C::TB];
+    constexpr int NT = 32 * (NAW + NBW), AT = 32 * NAW, BT = 32 * NBW;
+    const int tile = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const int a = tile / C::TILES_PER_A, b2base = (tile % C::TILES_PER_A) * C::G;
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTG; ++s) mbar_init(&full[s], 1);
+        for (int b = 0; b < 2; ++b) { mbar_init(&sready[b], NAW); mbar_init(&sfree[b], 1); }
+        mbar_fence_init();
+    }
+    for (int x = tid; x < C::TC; x += NT) s_twc[x] = g.twc[x];
+    for (int x = tid; x < C::TB; x += NT) s_twb[x] = g.twb[x];
+    __syncthreads();
+
+    if (tid < AT) {
+        // ------------------------------------------------------------------ line warps: A0, A1
+        constexpr int NI0 = ceil_div(C::ITEMS_LINE_Q, AT), NI1 = ceil_div(C::ITEMS_LINE_P, AT);
+        if (tid < 32) {
+            for (int t = 0; t < NSTG && t < g.count; ++t)
+                issue_operand_loads<C>(g, g.desc[t], OP + static_cast<size_t>(t) * C::OP_DOUBLES, &full[t], a, b2base, tid);
+            if (prefetch_operands<NSTG>() && NSTG < g.count) issue_operand_prefetch<C>(g, g.desc[NSTG], a, b2base, tid);
+        }
+        LineQIdx q0[NI0];
+        double vj[NI0][C::PCN], vl[NI0][C::PCN];
+#pragma unroll
+        for (int m = 0; m < NI0; ++m) {
+            const int w = tid + m * AT;
+            q0[m] = lineq_index<C, false>(w < C::ITEMS_LINE_Q ? w : 0, a, b2base);
+            const double* pj = g.psi_r + static_cast<size_t>(g.j) * g.m_points + q0[m].gofs;
+            const double* pl = g.psi_r + static_cast<size_t>(g.l >= 0 ? g.l : g.j) * g.m_points + q0[m].gofs;
+#pragma unroll
+            for (int n1 = 0; n1 < C::PCN; ++n1) { vj[m][n1] = ld_ro(pj + C::QC * n1); vl[m][n1] = ld_ro(pl + C::QC * n1); }
+        }
+        int flags_next = g.desc[0].flags;
+        for (int t = 0; t < g.count; ++t) {
+            const int s = t % NSTG, b = t & 1;
+            double2* const S = S0 + b * BUF;
+            double* stage = OP + static_cast<size_t>(s) * C::OP_DOUBLES;
+            const int flags = flags_next;
+            if (t + 1 < g.count) flags_next = g.desc[t + 1].flags;
+            if (t >= 2) mbar_wait(&sfree[b], ((t >> 1) - 1) & 1);      // the tile store of t-2 has read this buffer
+            mbar_wait(&full[s], (t / NSTG) & 1);
+#pragma unroll
+            for (int m = 0; m < NI0; ++m) {
+                const int w = tid + m * AT;
+                if (w < C::ITEMS_LINE_Q)
+                    a0_compute_ts<C>(vj[m], vl[m], stage + q0[m].op, flags, S + (w / C::QC) * C::TC, w / C::QC, q0[m].n2, s_twc + q0[m].n2);
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(AT) : "memory");
+            if (tid < 32 && t + NSTG < g.count) {                      // the stage has been consumed: refill it
+                issue_operand_loads<C>(g, g.desc[t + NSTG], stage, &full[s], a, b2base, tid);
+                if (prefetch_operands<NSTG>() && t + NSTG + 1 < g.count) issue_operand_prefetch<C>(g, g.desc[t + NSTG + 1], a, b2base, tid);
+            }
+#pragma unroll
+            for (int m = 0; m < NI1; ++m) {
+                const int w = tid + m * AT;                            // item (line, k1)
+                if (w < C::ITEMS_LINE_P) a1_compute_ts<C>(S + (w / C::PC) * C::TC + (w % C::PC) * C::QC, w & 7);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sready[b]);
+        }
+    } else {
+        // ------------------------------------------------------------------ column warps: A2 in place, tile store
+        const int bt = tid - AT;
+        constexpr int NI2 = ceil_div(C::ITEMS_POS, BT);
+        static_assert(C::ITEMS_POS % 32 == 0, "whole k1 segments per warp");
+        for (int t = 0; t < g.count; ++t) {
+            const int b = t & 1;
+            double2* const S = S0 + b * BUF;
+            mbar_wait(&sready[b], (t >> 1) & 1);
+#pragma unroll
+            for (int m = 0; m < NI2; ++m) {
+                const int p = bt + m * BT;                             // warp-uniform condition: BT and ITEMS_POS are multiples of 32
+                if (p < C::ITEMS_POS) {
+                    double xr[C::R1], xi[C::R1];
+                    a2_load_ts<C>(S, p / C::QC, p % C::QC, xr, xi);
+                    __syncwarp();                                      // every lane of the warp has read its column
+                    a2_store_ts<C>(xr, xi, s_twb + b2base * C::R1, S + p);
+                }
+            }
+            fence_proxy_async();                                       // the tile is read by the TMA below
+            asm volatile("bar.sync 2, %0;" ::"n"(BT) : "memory");
+            if (bt == 0) {
+                tensor5_s2g(gx.w1_map, 0, b2base, a, 0, t * C::R1, S);
+                bulk_commit();
+                bulk_wait_read_all();
+                mbar_arrive(&sfree[b]);
+            }
+        }
+        if (bt == 0) bulk_wait_all();
     }
 }
 
