@@ -58,6 +58,44 @@ def test_apply_to_matches_oracle(base, dims, n_occ, n_tgt, batch):
     plan.destroy()
 
 
+# ------------------------------------------------------------------ the TMA-tile kernels under the rectangular entry points
+@pytest.mark.parametrize("base,dims", [("C1", (16, 192, 192)), ("C1", (32, 64, 128)), ("C2", (8, 64, 128)), ("C2", (16, 96, 96))])
+def test_tma_tile_geometries_under_apply_to_block_and_complex(base, dims):
+    """Geometries whose pass C gathers its W1 tile by a TMA tensor-box copy (c-axis transform length 128 / 192 / 256, one b2 per
+    tile) and whose pass A (periodic) sends it by a tensor-box store, driven through exx_apply_to, exx_apply_block and
+    exx_apply_complex: resident and streamed sets differ, so the partner-set and accumulate paths of those kernels run too."""
+    n_a, n_b = 3, 2
+    w = make_workload(small_spec(base, dims=dims, n_orb=n_a + n_b + 1, spacing=(0.45, 0.4, 0.5), number=1900 + sum(dims)))
+    spec = w["spec"]
+    plan = exx.ExxPlan(spec.dims, spec.spacing, spec.bc, w["kernel"], max_orbitals=n_a + n_b + 1)
+    plan.set_batch(2)
+    o = Oracle(spec.dims, spec.spacing, spec.bc, w["kernel"])
+    allp = w["psi"].cuda()
+    pa, pb = allp[:n_a].contiguous(), allp[n_a:n_a + n_b].contiguous()
+    ha, hb = w["psi"][:n_a].numpy(), w["psi"][n_a:n_a + n_b].numpy()
+    occ_a, occ_b = np.array([2.0, 0.0, 1.3]), np.array([0.6, 1.0])
+    # apply_to
+    kphi = plan.apply_to(pa, occ_a, pb)
+    ref = o.apply_to(ha, occ_a, hb)
+    assert np.max(np.abs(kphi.cpu().numpy() - ref)) <= K_RTOL * np.max(np.abs(ref))
+    # apply_block
+    ka, kb = torch.empty_like(pa), torch.empty_like(pb)
+    ex = plan.apply_block(pa, occ_a, ka, pb, occ_b, kb)
+    ka_ref, kb_ref, ex_ref, _ = o.apply_block(ha, occ_a, hb, occ_b)
+    assert np.max(np.abs(ka.cpu().numpy() - ka_ref)) <= K_RTOL * np.max(np.abs(ka_ref))
+    assert np.max(np.abs(kb.cpu().numpy() - kb_ref)) <= K_RTOL * np.max(np.abs(kb_ref))
+    assert abs(ex - ex_ref) <= E_RTOL * abs(ex_ref)
+    # complex orbitals: 3 complex = 6 real
+    planar = w["psi"].reshape(2, 3, *dims)
+    occ_c = np.array([2.0, 0.9, 0.4])
+    k_ref, exc_ref = o.apply_complex(planar[0].numpy() + 1j * planar[1].numpy(), occ_c)
+    kpl, exc = plan.apply_complex(planar.cuda(), occ_c)
+    k_gpu = kpl[0].cpu().numpy() + 1j * kpl[1].cpu().numpy()
+    assert np.max(np.abs(k_gpu - k_ref)) <= K_RTOL * np.max(np.abs(k_ref))
+    assert abs(exc - exc_ref) <= E_RTOL * abs(exc_ref)
+    plan.destroy()
+
+
 # ------------------------------------------------------------------ NEXT-1: complex orbitals
 @pytest.mark.parametrize("base,dims,n_orb,batch", [("C1", (16, 16, 16), 3, 0), ("C2", (8, 16, 8), 3, 2), ("C1", (96, 96, 96), 3, 3),
                                                    ("C2", (48, 48, 48), 2, 0)])
