@@ -57,3 +57,35 @@ def test_single_rank_is_identity():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.aggregate_over_ranks(50.0, 36, 1) == (50.0, pytest.approx(36 / 0.05))
+
+
+def test_rank_plumbing_and_step_counts(monkeypatch):
+    """bench.py's launch plumbing without a GPU: under torchrun the ranks come from the environment; a plain
+    `python bench.py --gpus N` (WORLD_SIZE unset) must spawn its N ranks itself; the driver's --steps / --warmup are
+    honoured up to the per-configuration caps and never fall below three warm-up steps."""
+    sys.path.insert(0, ROOT)
+    import bench
+    for k in ("WORLD_SIZE", "RANK", "LOCAL_RANK"):
+        monkeypatch.delenv(k, raising=False)
+    assert bench.rank_env(1) == (0, 0, 1, False)
+    assert bench.rank_env(8) == (0, 0, 1, True)                  # nobody launched the ranks: bench spawns them
+    monkeypatch.setenv("WORLD_SIZE", "4")
+    monkeypatch.setenv("RANK", "3")
+    monkeypatch.setenv("LOCAL_RANK", "3")
+    assert bench.rank_env(4) == (3, 3, 4, False)
+    assert bench.effective_counts("C5", None, 3) == (2, 3)
+    assert bench.effective_counts("C5", 20, 5) == (2, 3)         # capped: a C5 apply takes the better part of a minute
+    assert bench.effective_counts("C3", 20, 1) == (20, 3)        # at least three warm-up steps
+    assert bench.effective_counts("C3", 1000, 50) == (50, 5)
+    assert bench.effective_counts("C4", None, 3, quick=True) == (1, 1)
+
+
+def test_reference_arm_exits_quietly_on_other_ranks(monkeypatch, capsys):
+    """--impl reference under torchrun: rank 0 alone runs the oracle; the other ranks return without work or output."""
+    sys.path.insert(0, ROOT)
+    import argparse
+
+    import bench
+    args = argparse.Namespace(config="C1", steps=1, warmup=1, gpus=2)
+    bench.run_reference(args, rank=1, world=2)
+    assert capsys.readouterr().out == ""
