@@ -209,7 +209,10 @@ struct TuneB {
     // to feed both kinds of warps: WS with two full work buffers, else (free BC) WSF with NA-row buffers and per-warp
     // expansion scratch; else work + landing buffer with CTA barriers
     static constexpr int NY = Cfg::NGRP <= 12 ? Cfg::NGRP : Cfg::NGRP / 2;       // column warps
-    static constexpr int NX = 4;                                                // row warps (2, 3, 5, 6 measured slower)
+    // row warps: 4 (2, 3, 5, 6 measured slower at 96^3 and 256^3 free); 6 where eight column warps leave the registers for
+    // them and the (a, pin) items of a block split evenly over 192 threads (192^3: pass B -5.5 %, measured after B4 had
+    // become an in-place stage + TMA row stores)
+    static constexpr int NX = (!FREE && NY == 8 && Cfg::ITEMS_IO % 192 == 0) ? 6 : 4;
     static constexpr bool kBig = Cfg::NGRP >= 6 && (Cfg::NGRP <= 12 || Cfg::NGRP % 2 == 0);
     static constexpr int SMEM_WS = (2 * Cfg::WORK_ELEMS + 2 * TA) * 16;
     static constexpr int SMEM_WSF = (2 * Cfg::P_ELEMS + NY * Cfg::E_ELEMS + 2 * TA) * 16;
